@@ -1,0 +1,339 @@
+/*
+ * oracle.c -- plain, slow, CPU reference of the KBMOD shift-and-stack hot path.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call this file.  The product
+ * (paper_1901_02492_b200/) never links, imports or falls back to it, and it shares no
+ * code, headers, tables or helpers with the CUDA path.
+ *
+ * Every function below is the paper's definition written as nested loops (citations are
+ * PAPER.md line numbers, "P:<line>").  Readings of silent/garbled passages are the ones
+ * listed in DESIGN.md ("Readings", R1..R14).  Pins that check this file against
+ * something other than itself live in tests/test_oracle_pins.py (all pinned: P1 analytic
+ * source, P2 N(0,1) noise statistics, P3 v=0 inverse-variance coadd vs numpy.average,
+ * P4 independent brute force, P5 index-revealing images, P6 mask invariants, P7 scalings).
+ *
+ * Build: gcc -O2 -std=c99 -ffp-contract=off -fopenmp -shared -fPIC oracle.c -lm
+ *   -ffp-contract=off matters: positions and f32seq sums are defined as separately
+ *   rounded binary32 operations (R8, R9); an FMA would change them.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_OK 0
+#define ORACLE_ERR_ARG (-3)
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* A pixel carries information iff it is unmasked and numerically usable.
+ * P:171 "we set the inverse variance to zero so that they will add nothing to the
+ * likelihood sum"; non-finite or non-positive variance is read the same way (R6). */
+static int good_pixel(const float* sci, const float* var, const uint8_t* mask, size_t k) {
+    if (mask && mask[k]) return 0;
+    if (!isfinite(sci[k]) || !isfinite(var[k])) return 0;
+    return var[k] > 0.0f;
+}
+
+/*
+ * O1. Likelihood images, diagonal covariance.  P:161-167 Eq.19-20:
+ *     Psi(y) = sum_x n(x) T(x - y) / sigma^2(x)
+ *     Phi(y) = sum_x T(x - y)^2    / sigma^2(x)
+ * written with d = x - y over the P x P support of T: a cross-correlation (R2), terms
+ * outside the image or on a not-good pixel have inverse variance 0 (R4, R5).
+ * Sums in double, stored as binary32.  If the centre pixel itself is not good, or
+ * Phi <= 0, the pixel holds the invalid marker (psi = NaN, phi = 0) (R4).
+ *
+ * psf[i][r+dy][r+dx] = T_i(dx, dy).  psiphi is [N,H,W,2] (psi, phi interleaved).
+ * psi_abs (optional, may be NULL): sum of |terms| of Psi, for the parity tolerance.
+ */
+int oracle_make_psi_phi(const float* sci, const float* var, const uint8_t* mask,
+                        const float* psf, int N, int H, int W, int P,
+                        float* psiphi, float* psi_abs) {
+    if (!sci || !var || !psf || !psiphi) return ORACLE_ERR_ARG;
+    if (N <= 0 || H <= 0 || W <= 0 || P <= 0 || (P % 2) == 0) return ORACLE_ERR_ARG;
+    const int r = (P - 1) / 2;
+    for (int i = 0; i < N; ++i) {
+        const size_t off = (size_t)i * H * W;
+        const float* s = sci + off;
+        const float* v = var + off;
+        const uint8_t* m = mask ? mask + off : NULL;
+        const float* T = psf + (size_t)i * P * P;
+#pragma omp parallel for schedule(static)
+        for (int y = 0; y < H; ++y) {
+            for (int x = 0; x < W; ++x) {
+                double psi = 0.0, phi = 0.0, pabs = 0.0;
+                for (int dy = -r; dy <= r; ++dy) {
+                    const int yy = y + dy;
+                    if (yy < 0 || yy >= H) continue;
+                    for (int dx = -r; dx <= r; ++dx) {
+                        const int xx = x + dx;
+                        if (xx < 0 || xx >= W) continue;
+                        const size_t k = (size_t)yy * W + xx;
+                        if (!good_pixel(s, v, m, k)) continue;
+                        const double t = (double)T[(dy + r) * P + (dx + r)];
+                        const double term = (double)s[k] / (double)v[k] * t;
+                        psi += term;
+                        pabs += fabs(term);
+                        phi += (1.0 / (double)v[k]) * t * t;
+                    }
+                }
+                const size_t c = (size_t)y * W + x;
+                float fpsi = (float)psi, fphi = (float)phi;
+                if (!good_pixel(s, v, m, c) || !(fphi > 0.0f)) {
+                    fpsi = NAN;
+                    fphi = 0.0f;
+                }
+                psiphi[2 * (off + c)] = fpsi;
+                psiphi[2 * (off + c) + 1] = fphi;
+                if (psi_abs) psi_abs[off + c] = (float)pabs;
+            }
+        }
+    }
+    return ORACLE_OK;
+}
+
+/*
+ * S3. Pixel hit by a linear trajectory (P:203 linear trajectories; start pixel in the
+ * first image P:231; nearest pixel, R8/R9):
+ *     f  = fl( fl(p0) + fl(v * dt) )          three separately rounded binary32 ops
+ *     ip = floor( fl(f + 0.5f) )              exact halves round up
+ * Returns 0 and leaves *ip alone when the pixel is outside [0, n).
+ */
+static int traj_pixel(int p0, float v, float dt, int n, int* ip) {
+    volatile float prod = v * dt;
+    volatile float f = (float)p0 + prod;
+    volatile float g = f + 0.5f;
+    const float fl = floorf(g);
+    if (!(fl >= 0.0f && fl < (float)n)) return 0;
+    *ip = (int)fl;
+    return 1;
+}
+
+typedef struct {
+    float Psi, Phi;
+    int n_obs;
+} coadd_t;
+
+/*
+ * S4. Coadded likelihood along one trajectory.  P:193-195 Eq.24-25:
+ *     Psi_coadd = sum_i Psi_i(y_i),  Phi_coadd = sum_i Phi_i(y_i)
+ * over the observations that exist: in bounds and not the invalid marker.
+ * Images in order i = 0..N-1.  mode 0 ("f64"): sums in double, rounded once to binary32.
+ * mode 1 ("f32seq"): binary32 adds in image order (R13).
+ * ixiy (optional): per-image pixel, (-1,-1) when out of bounds.
+ */
+static coadd_t coadd(const float* psiphi, const float* dt, int N, int H, int W,
+                     int x0, int y0, float vx, float vy, int mode, int* ixiy) {
+    double dPsi = 0.0, dPhi = 0.0;
+    float fPsi = 0.0f, fPhi = 0.0f;
+    int n = 0;
+    for (int i = 0; i < N; ++i) {
+        int ix = -1, iy = -1;
+        const int inx = traj_pixel(x0, vx, dt[i], W, &ix);
+        const int iny = traj_pixel(y0, vy, dt[i], H, &iy);
+        if (ixiy) {
+            ixiy[2 * i] = (inx && iny) ? ix : -1;
+            ixiy[2 * i + 1] = (inx && iny) ? iy : -1;
+        }
+        if (!(inx && iny)) continue;
+        const size_t k = 2 * (((size_t)i * H + iy) * W + ix);
+        const float psi = psiphi[k], phi = psiphi[k + 1];
+        if (isnan(psi)) continue;
+        if (mode == 0) {
+            dPsi += (double)psi;
+            dPhi += (double)phi;
+        } else {
+            volatile float a = fPsi + psi;
+            volatile float b = fPhi + phi;
+            fPsi = a;
+            fPhi = b;
+        }
+        ++n;
+    }
+    coadd_t c;
+    c.Psi = (mode == 0) ? (float)dPsi : fPsi;
+    c.Phi = (mode == 0) ? (float)dPhi : fPhi;
+    c.n_obs = n;
+    return c;
+}
+
+static void make_dt(const double* times, int N, float* dt) {
+    /* R7: differenced in double against image 0, rounded once to binary32 */
+    for (int i = 0; i < N; ++i) dt[i] = (float)(times[i] - times[0]);
+}
+
+/* S5. P:180 Eq.22 alpha = Psi/Phi; Eq.26 nu = Psi/sqrt(Phi) (R1).
+ * binary32, correctly rounded sqrt and divisions. */
+static void score(coadd_t c, float* nu, float* alpha) {
+    volatile float s = sqrtf(c.Phi);
+    volatile float q = c.Psi / s;
+    volatile float a = c.Psi / c.Phi;
+    *nu = q;
+    *alpha = a;
+}
+
+typedef struct {
+    float nu;
+    int j;
+} cand_t;
+
+/* larger nu first; equal nu: smaller velocity index first (R11) */
+static int cand_cmp(const void* pa, const void* pb) {
+    const cand_t* a = (const cand_t*)pa;
+    const cand_t* b = (const cand_t*)pb;
+    if (a->nu > b->nu) return -1;
+    if (a->nu < b->nu) return 1;
+    return (a->j > b->j) - (a->j < b->j);
+}
+
+/*
+ * O2. Exhaustive search.  P:205 Eq.27 argmax over (y0, v) of nu_coadd; "evaluate
+ * nu for all possible values of y0 and v"; P:231 every start pixel of the first image x
+ * every grid velocity.  Retention: the K eligible trajectories of largest nu per start
+ * pixel (BASELINE.json north_star; R10), eligible <=> n_obs >= min_obs and Phi > 0.
+ * Selection by a full sort of all V candidates.
+ * Output planes are [(y_end - y_begin), W, K]; empty slots: vel_idx = -1, n_obs = 0,
+ * psi = phi = alpha = 0, nu = -inf (R12).
+ */
+int oracle_search(const float* psiphi, const double* times, int N, int H, int W,
+                  const float* vel, int V, int K, int min_obs, int mode,
+                  int y_begin, int y_end,
+                  int32_t* o_vel, int32_t* o_nobs, float* o_psi, float* o_phi,
+                  float* o_nu, float* o_alpha) {
+    if (!psiphi || !times || !vel || !o_vel || !o_nobs || !o_psi || !o_phi || !o_nu || !o_alpha)
+        return ORACLE_ERR_ARG;
+    if (N <= 0 || H <= 0 || W <= 0 || V <= 0 || K <= 0 || min_obs < 1) return ORACLE_ERR_ARG;
+    if (y_begin < 0 || y_end > H || y_begin > y_end) return ORACLE_ERR_ARG;
+    float* dt = (float*)malloc(sizeof(float) * N);
+    make_dt(times, N, dt);
+    int err = 0;
+#pragma omp parallel
+    {
+        cand_t* cand = (cand_t*)malloc(sizeof(cand_t) * V);
+        coadd_t* acc = (coadd_t*)malloc(sizeof(coadd_t) * V);
+        if (!cand || !acc) {
+#pragma omp atomic write
+            err = 1;
+        }
+#pragma omp for schedule(dynamic, 1)
+        for (int y0 = y_begin; y0 < y_end; ++y0) {
+            if (!cand || !acc) continue;
+            for (int x0 = 0; x0 < W; ++x0) {
+                int nc = 0;
+                for (int j = 0; j < V; ++j) {
+                    acc[j] = coadd(psiphi, dt, N, H, W, x0, y0, vel[2 * j], vel[2 * j + 1], mode, NULL);
+                    if (acc[j].n_obs >= min_obs && acc[j].Phi > 0.0f) {
+                        float nu, alpha;
+                        score(acc[j], &nu, &alpha);
+                        cand[nc].nu = nu;
+                        cand[nc].j = j;
+                        ++nc;
+                    }
+                }
+                qsort(cand, nc, sizeof(cand_t), cand_cmp);
+                const size_t base = ((size_t)(y0 - y_begin) * W + x0) * K;
+                for (int k = 0; k < K; ++k) {
+                    if (k < nc) {
+                        const int j = cand[k].j;
+                        float nu, alpha;
+                        score(acc[j], &nu, &alpha);
+                        o_vel[base + k] = j;
+                        o_nobs[base + k] = acc[j].n_obs;
+                        o_psi[base + k] = acc[j].Psi;
+                        o_phi[base + k] = acc[j].Phi;
+                        o_nu[base + k] = nu;
+                        o_alpha[base + k] = alpha;
+                    } else {
+                        o_vel[base + k] = -1;
+                        o_nobs[base + k] = 0;
+                        o_psi[base + k] = 0.0f;
+                        o_phi[base + k] = 0.0f;
+                        o_nu[base + k] = -INFINITY;
+                        o_alpha[base + k] = 0.0f;
+                    }
+                }
+            }
+        }
+        free(cand);
+        free(acc);
+    }
+    free(dt);
+    return err ? ORACLE_ERR_ARG : ORACLE_OK;
+}
+
+/* O3. Dense evaluation: Psi, Phi, n_obs for every (start pixel, velocity) of a row band.
+ * Planes [(y_end - y_begin), W, V].  Same loops as O2 without S5/S6. */
+int oracle_eval_all(const float* psiphi, const double* times, int N, int H, int W,
+                    const float* vel, int V, int mode, int y_begin, int y_end,
+                    float* Psi, float* Phi, int32_t* n_obs) {
+    if (!psiphi || !times || !vel || !Psi || !Phi || !n_obs) return ORACLE_ERR_ARG;
+    if (N <= 0 || H <= 0 || W <= 0 || V <= 0) return ORACLE_ERR_ARG;
+    if (y_begin < 0 || y_end > H || y_begin > y_end) return ORACLE_ERR_ARG;
+    float* dt = (float*)malloc(sizeof(float) * N);
+    make_dt(times, N, dt);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int y0 = y_begin; y0 < y_end; ++y0)
+        for (int x0 = 0; x0 < W; ++x0)
+            for (int j = 0; j < V; ++j) {
+                const coadd_t c = coadd(psiphi, dt, N, H, W, x0, y0, vel[2 * j], vel[2 * j + 1], mode, NULL);
+                const size_t k = ((size_t)(y0 - y_begin) * W + x0) * V + j;
+                Psi[k] = c.Psi;
+                Phi[k] = c.Phi;
+                n_obs[k] = c.n_obs;
+            }
+    free(dt);
+    return ORACLE_OK;
+}
+
+/* Explicit trajectory list: x0y0 [M,2] int, vxvy [M,2] float -> Psi, Phi, n_obs [M],
+ * ixiy [M,N,2] (optional; (-1,-1) where the trajectory leaves the image). */
+int oracle_eval_trajectories(const float* psiphi, const double* times, int N, int H, int W,
+                             const int32_t* x0y0, const float* vxvy, int M, int mode,
+                             float* Psi, float* Phi, int32_t* n_obs, int32_t* ixiy) {
+    if (!psiphi || !times || !x0y0 || !vxvy || !Psi || !Phi || !n_obs) return ORACLE_ERR_ARG;
+    if (N <= 0 || H <= 0 || W <= 0 || M < 0) return ORACLE_ERR_ARG;
+    float* dt = (float*)malloc(sizeof(float) * N);
+    make_dt(times, N, dt);
+    for (int m = 0; m < M; ++m) {
+        const coadd_t c = coadd(psiphi, dt, N, H, W, x0y0[2 * m], x0y0[2 * m + 1],
+                                vxvy[2 * m], vxvy[2 * m + 1], mode,
+                                ixiy ? ixiy + (size_t)m * N * 2 : NULL);
+        Psi[m] = c.Psi;
+        Phi[m] = c.Phi;
+        n_obs[m] = c.n_obs;
+    }
+    free(dt);
+    return ORACLE_OK;
+}
+
+/* S5 for arrays (used by the pins to score dense evaluations). */
+int oracle_score(const float* Psi, const float* Phi, size_t n, float* nu, float* alpha) {
+    if (!Psi || !Phi || !nu || !alpha) return ORACLE_ERR_ARG;
+    for (size_t k = 0; k < n; ++k) {
+        coadd_t c;
+        c.Psi = Psi[k];
+        c.Phi = Phi[k];
+        c.n_obs = 0;
+        score(c, &nu[k], &alpha[k]);
+    }
+    return ORACLE_OK;
+}
