@@ -1,0 +1,150 @@
+/*
+ * kbmod_b200.h -- C ABI of the B200-native KBMOD shift-and-stack hot path.
+ *
+ * The calls follow the paper's statement of the problem (Whidden et al. 2019,
+ * arXiv:1901.02492; citations below are PAPER.md line numbers "P:<line>"):
+ *   1. kbmod_make_psi_phi : per-image likelihood images Psi_i, Phi_i   (Eq.19-20)
+ *   2. kbmod_search       : exhaustive linear-trajectory search        (Eq.24-27)
+ * plus a test hook (kbmod_eval_trajectories) and small utilities.
+ *
+ * Conventions
+ *   - Plain C, no torch / C++ types.  Pointers are DEVICE pointers unless marked HOST.
+ *   - The library never allocates or frees caller-visible memory and never synchronises the
+ *     stream.  The caller (PyTorch in this repo) owns every buffer and the stream.  HOST
+ *     arrays are consumed before the call returns.
+ *   - Images are row-major [N][H][W], x (column) fastest.  Integer coordinates are pixel
+ *     centres; pixel ix covers [ix-0.5, ix+0.5).
+ *   - Return value: KBMOD_OK (0) or a negative kbmod_status.  Argument errors are found
+ *     before any launch; asynchronous faults surface at the caller's next synchronisation.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns
+ *     KBMOD_ERR_CUDA.
+ */
+#ifndef KBMOD_B200_H
+#define KBMOD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    KBMOD_OK = 0,
+    KBMOD_ERR_NULL = -1,        /* a required pointer is NULL */
+    KBMOD_ERR_SHAPE = -2,       /* non-positive or inconsistent dimension */
+    KBMOD_ERR_ARG = -3,         /* value out of range (even P, K, min_obs, non-finite time ...) */
+    KBMOD_ERR_ALIGN = -4,       /* pointer not aligned as documented */
+    KBMOD_ERR_CUDA = -5,        /* CUDA runtime error at launch / no device */
+    KBMOD_ERR_UNSUPPORTED = -6, /* beyond the supported limits (P > 31, N > 64, K > 32) */
+    KBMOD_ERR_WORKSPACE = -7    /* workspace smaller than kbmod_search_workspace() */
+} kbmod_status;
+
+#define KBMOD_MAX_PSF 31
+#define KBMOD_MAX_IMAGES 64
+#define KBMOD_MAX_K 32
+
+/* Result planes of kbmod_search (structure of arrays).  Each member is a DEVICE pointer to
+ * [H][W][K] elements, caller-owned.  For one start pixel the K slots are sorted by nu
+ * descending (ties: smaller vel_idx first).  Unused slots: vel_idx = -1, n_obs = 0,
+ * psi = phi = alpha = 0, nu = -INFINITY.  (Candidate record of P:241-249: start pixel =
+ * plane position, velocity = vel_grid[vel_idx], likelihood nu, flux alpha.) */
+typedef struct {
+    int32_t* vel_idx;
+    int32_t* n_obs;
+    float* psi;    /* Psi_coadd, Eq.24 */
+    float* phi;    /* Phi_coadd, Eq.25 */
+    float* nu;     /* Psi/sqrt(Phi), Eq.26 */
+    float* alpha;  /* Psi/Phi, Eq.22 */
+} kbmod_result;
+
+/*
+ * Likelihood images with diagonal covariance (Eq.19-20):
+ *     Psi_i(y) = sum_d  sci_i(y+d)/var_i(y+d) * T_i(d)
+ *     Phi_i(y) = sum_d        1/var_i(y+d)    * T_i(d)^2       d over the P x P support
+ * A pixel has zero inverse variance when it is masked, when sci or var is not finite, when
+ * var <= 0, or when it lies outside the image.  If the centre pixel itself has zero
+ * inverse variance (or Phi <= 0) the output is the invalid marker (psi = NaN, phi = 0).
+ * This is a cross-correlation with T (Eq.19), not a convolution; they coincide for
+ * point-symmetric kernels.  Arithmetic: fp32 FMAs.
+ *
+ *   sci, var : [N][H][W] float, device
+ *   mask     : [N][H][W] uint8, device, nonzero = masked; may be NULL (no mask)
+ *   psf      : HOST [N][P][P] float, psf[i][r+dy][r+dx] = T_i(dx,dy), r = (P-1)/2; taken as
+ *              given (any values, not renormalised); copied before return
+ *   P        : odd, 1 <= P <= KBMOD_MAX_PSF
+ *   psiphi   : out, [N][H][W][2] float (psi, phi interleaved: one 8-byte sample),
+ *              device, 8-byte aligned; must not alias the inputs
+ *   stream   : cudaStream_t (NULL = default stream)
+ */
+int kbmod_make_psi_phi(const float* sci, const float* var, const uint8_t* mask,
+                       const float* psf, int N, int H, int W, int P,
+                       float* psiphi, void* stream);
+
+/*
+ * Exhaustive search (Eq.27).  For every start pixel (x0,y0) of image 0
+ * and every velocity j of vel_grid:
+ *     dt_i = (float)(times[i] - times[0])
+ *     ix   = floor( fl( fl( fl(x0) + fl(vx_j*dt_i) ) + 0.5f ) )     (same for y; binary32,
+ *            round-to-nearest-even, never fused; exact halves round up)
+ *     an observation exists iff 0<=ix<W, 0<=iy<H and psi_i[iy][ix] is not NaN
+ *     Psi = sum psi_i[iy][ix], Phi = sum phi_i[iy][ix]   fp32 adds, images in order 0..N-1
+ *     eligible iff n_obs >= min_obs and Phi > 0
+ *     nu = Psi/sqrt(Phi), alpha = Psi/Phi                 correctly rounded fp32
+ * and the K eligible trajectories of largest nu are kept per start pixel (see kbmod_result).
+ *
+ *   psiphi    : [N][H][W][2] float as produced above, device, 16-byte aligned.  Contract: phi
+ *               is finite and >= 0 wherever psi is not NaN; psi is finite or NaN.
+ *   times     : HOST [N] double, days, finite; need not be sorted; times[0] is the start image
+ *   vel_grid  : HOST [V][2] float (vx, vy) px/day, finite
+ *   V >= 1; 1 <= K <= KBMOD_MAX_K; 1 <= min_obs <= N; 1 <= N <= KBMOD_MAX_IMAGES
+ *   out       : HOST struct of DEVICE plane pointers, each [H][W][K], 4-byte aligned
+ *   workspace : device scratch of at least kbmod_search_workspace(N,H,W,V,K) bytes,
+ *               256-byte aligned; contents undefined afterwards
+ */
+int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
+                 const float* vel_grid, int V, int K, int min_obs,
+                 const kbmod_result* out, void* workspace, size_t workspace_bytes,
+                 void* stream);
+
+/* Bytes of device scratch kbmod_search needs for these sizes (pure function; 0 on bad sizes). */
+size_t kbmod_search_workspace(int N, int H, int W, int V, int K);
+
+/* As kbmod_search with psi and phi given as two separate [N][H][W] float planes (the literal
+ * signature of the problem statement).  They are interleaved into the workspace first, so the
+ * workspace must hold kbmod_search_workspace(...) + N*H*W*8 bytes. */
+int kbmod_search_split(const float* psi, const float* phi, const double* times, int N, int H,
+                       int W, const float* vel_grid, int V, int K, int min_obs,
+                       const kbmod_result* out, void* workspace, size_t workspace_bytes,
+                       void* stream);
+
+/*
+ * Test hook: evaluate an explicit list of M trajectories with exactly the arithmetic of
+ * kbmod_search (S3 + S4), returning the coadds and every sampled pixel.
+ *   x0y0 : [M][2] int32 device;  vxvy : [M][2] float device;  times : HOST [N] double
+ *   Psi, Phi : [M] float device;  n_obs : [M] int32 device
+ *   ixiy : [M][N][2] int32 device or NULL; (-1,-1) where the trajectory is off the image
+ */
+int kbmod_eval_trajectories(const float* psiphi, const double* times, int N, int H, int W,
+                            const int32_t* x0y0, const float* vxvy, int M,
+                            float* Psi, float* Phi, int32_t* n_obs, int32_t* ixiy,
+                            void* stream);
+
+/* Selects the search kernel: 0 = automatic (default), 1 = direct-gather kernel (global loads,
+ * any shape), 2 = shared-memory staged kernel (KBMOD_ERR_UNSUPPORTED from kbmod_search if the
+ * shape does not fit it).  Process-wide; for tests and benchmarks. */
+int kbmod_set_search_kernel(int which);
+
+/* Number of kernel launches issued by this library since load (for benchmark accounting). */
+unsigned long long kbmod_launch_count(void);
+
+/* Static description of a status code. */
+const char* kbmod_status_string(int status);
+
+/* Library version, "major.minor". */
+const char* kbmod_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KBMOD_B200_H */

@@ -1,0 +1,189 @@
+"""Thin Python binding of libkbmod_b200.so (include/kbmod_b200.h).
+
+Argument marshalling only: every step of the path runs in the library's CUDA kernels.  PyTorch
+supplies device memory and the stream.  There is no CPU fallback: if the library cannot be
+loaded, or a compute call is made without a CUDA device, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Dict, Optional
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libkbmod_b200.so")
+_lib: Optional[ctypes.CDLL] = None
+
+EXPORTS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_workspace", "kbmod_search_split",
+           "kbmod_eval_trajectories", "kbmod_set_search_kernel", "kbmod_launch_count",
+           "kbmod_status_string", "kbmod_version")
+
+
+class KbmodError(RuntimeError):
+    pass
+
+
+class _Result(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")]
+
+
+def lib() -> ctypes.CDLL:
+    """Loads the in-tree C-ABI library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise KbmodError(f"{LIB_PATH} is missing: run paper_1901_02492_b200/build.py "
+                             "(or __graft_entry__.build()); there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        L.kbmod_search_workspace.restype = ctypes.c_size_t
+        L.kbmod_launch_count.restype = ctypes.c_ulonglong
+        L.kbmod_status_string.restype = ctypes.c_char_p
+        L.kbmod_version.restype = ctypes.c_char_p
+        for n in ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_split",
+                  "kbmod_eval_trajectories", "kbmod_set_search_kernel"):
+            getattr(L, n).restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        raise KbmodError(f"{what} failed: {rc} ({lib().kbmod_status_string(rc).decode()})")
+
+
+def _dev(t: Optional[torch.Tensor], dtype, what: str):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise KbmodError(f"{what}: expected a contiguous CUDA tensor of {dtype}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _host(a, dtype) -> np.ndarray:
+    if isinstance(a, torch.Tensor):
+        a = a.detach().cpu().numpy()
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _stream() -> ctypes.c_void_p:
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def version() -> str:
+    return lib().kbmod_version().decode()
+
+
+def launch_count() -> int:
+    return int(lib().kbmod_launch_count())
+
+
+def set_search_kernel(which: int) -> None:
+    _check(lib().kbmod_set_search_kernel(int(which)), "kbmod_set_search_kernel")
+
+
+def search_workspace(N: int, H: int, W: int, V: int, K: int) -> int:
+    return int(lib().kbmod_search_workspace(N, H, W, V, K))
+
+
+def make_psi_phi(sci: torch.Tensor, var: torch.Tensor, mask: Optional[torch.Tensor], psf,
+                 out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """kbmod_make_psi_phi: sci/var [N,H,W] f32 cuda, mask [N,H,W] u8 cuda or None, psf host
+    [N,P,P] -> psiphi [N,H,W,2] f32 cuda."""
+    N, H, W = sci.shape
+    psf = _host(psf, np.float32)
+    if psf.ndim != 3 or psf.shape[0] != N or psf.shape[1] != psf.shape[2]:
+        raise KbmodError("psf must be [N,P,P]")
+    if var.shape != sci.shape or (mask is not None and mask.shape != sci.shape):
+        raise KbmodError("sci, var, mask shapes differ")
+    if out is None:
+        out = torch.empty((N, H, W, 2), dtype=torch.float32, device=sci.device)
+    rc = lib().kbmod_make_psi_phi(_dev(sci, torch.float32, "sci"), _dev(var, torch.float32, "var"),
+                                  _dev(mask, torch.uint8, "mask"),
+                                  psf.ctypes.data_as(ctypes.c_void_p), N, H, W, psf.shape[1],
+                                  _dev(out, torch.float32, "psiphi"), _stream())
+    _check(rc, "kbmod_make_psi_phi")
+    return out
+
+
+def alloc_result(H: int, W: int, K: int, device) -> Dict[str, torch.Tensor]:
+    r = {k: torch.empty((H, W, K), dtype=torch.int32, device=device) for k in ("vel_idx", "n_obs")}
+    r.update({k: torch.empty((H, W, K), dtype=torch.float32, device=device)
+              for k in ("psi", "phi", "nu", "alpha")})
+    return r
+
+
+def search(psiphi: torch.Tensor, times, vel_grid, K: int, min_obs: int,
+           out: Optional[Dict[str, torch.Tensor]] = None,
+           workspace: Optional[torch.Tensor] = None) -> Dict[str, torch.Tensor]:
+    """kbmod_search: psiphi [N,H,W,2] f32 cuda, times host [N] f64, vel_grid host [V,2] f32."""
+    N, H, W, two = psiphi.shape
+    if two != 2:
+        raise KbmodError("psiphi must be [N,H,W,2]")
+    times = _host(times, np.float64)
+    vel = _host(vel_grid, np.float32)
+    if times.shape != (N,) or vel.ndim != 2 or vel.shape[1] != 2:
+        raise KbmodError("times must be [N], vel_grid [V,2]")
+    V = vel.shape[0]
+    if out is None:
+        out = alloc_result(H, W, K, psiphi.device)
+    need = search_workspace(N, H, W, V, K)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=psiphi.device)
+    res = _Result(*[ctypes.c_void_p(out[k].data_ptr()) for k in
+                    ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")])
+    for k in ("vel_idx", "n_obs"):
+        _dev(out[k], torch.int32, k)
+    for k in ("psi", "phi", "nu", "alpha"):
+        _dev(out[k], torch.float32, k)
+    rc = lib().kbmod_search(_dev(psiphi, torch.float32, "psiphi"),
+                            times.ctypes.data_as(ctypes.c_void_p), N, H, W,
+                            vel.ctypes.data_as(ctypes.c_void_p), V, int(K), int(min_obs),
+                            ctypes.byref(res), _dev(workspace, torch.uint8, "workspace"),
+                            ctypes.c_size_t(workspace.numel()), _stream())
+    _check(rc, "kbmod_search")
+    return out
+
+
+def search_split(psi: torch.Tensor, phi: torch.Tensor, times, vel_grid, K: int, min_obs: int):
+    """kbmod_search_split: psi, phi as separate [N,H,W] f32 cuda planes."""
+    N, H, W = psi.shape
+    times = _host(times, np.float64)
+    vel = _host(vel_grid, np.float32)
+    V = vel.shape[0]
+    out = alloc_result(H, W, K, psi.device)
+    need = search_workspace(N, H, W, V, K) + N * H * W * 8
+    ws = torch.empty(need, dtype=torch.uint8, device=psi.device)
+    res = _Result(*[ctypes.c_void_p(out[k].data_ptr()) for k in
+                    ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")])
+    rc = lib().kbmod_search_split(_dev(psi, torch.float32, "psi"), _dev(phi, torch.float32, "phi"),
+                                  times.ctypes.data_as(ctypes.c_void_p), N, H, W,
+                                  vel.ctypes.data_as(ctypes.c_void_p), V, int(K), int(min_obs),
+                                  ctypes.byref(res), _dev(ws, torch.uint8, "workspace"),
+                                  ctypes.c_size_t(ws.numel()), _stream())
+    _check(rc, "kbmod_search_split")
+    return out
+
+
+def eval_trajectories(psiphi: torch.Tensor, times, x0y0: torch.Tensor, vxvy: torch.Tensor,
+                      want_pixels: bool = True):
+    """kbmod_eval_trajectories (test hook) -> Psi, Phi, n_obs, ixiy (or None)."""
+    N, H, W, _ = psiphi.shape
+    times = _host(times, np.float64)
+    M = x0y0.shape[0]
+    dev = psiphi.device
+    Psi = torch.empty(M, dtype=torch.float32, device=dev)
+    Phi = torch.empty(M, dtype=torch.float32, device=dev)
+    nobs = torch.empty(M, dtype=torch.int32, device=dev)
+    ixiy = torch.empty((M, N, 2), dtype=torch.int32, device=dev) if want_pixels else None
+    rc = lib().kbmod_eval_trajectories(_dev(psiphi, torch.float32, "psiphi"),
+                                       times.ctypes.data_as(ctypes.c_void_p), N, H, W,
+                                       _dev(x0y0, torch.int32, "x0y0"),
+                                       _dev(vxvy, torch.float32, "vxvy"), M,
+                                       _dev(Psi, torch.float32, "Psi"), _dev(Phi, torch.float32, "Phi"),
+                                       _dev(nobs, torch.int32, "n_obs"),
+                                       _dev(ixiy, torch.int32, "ixiy"), _stream())
+    _check(rc, "kbmod_eval_trajectories")
+    return Psi, Phi, nobs, ixiy

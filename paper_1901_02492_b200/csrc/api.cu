@@ -1,0 +1,166 @@
+// api.cu -- the C ABI of include/kbmod_b200.h: argument checks, host-side tables, dispatch.
+#include <atomic>
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "common.cuh"
+#include "search_staged.cuh"
+
+namespace kbmod {
+static std::atomic<unsigned long long> g_launches{0};
+static std::atomic<int> g_search_kernel{0};
+void note_launch(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static int make_dt(const double* times, int N, DtTable& t) {
+    for (int i = 0; i < KBMOD_MAX_IMAGES; ++i) t.dt[i] = 0.0f;
+    for (int i = 0; i < N; ++i) {
+        if (!std::isfinite(times[i])) return KBMOD_ERR_ARG;
+        t.dt[i] = (float)(times[i] - times[0]);     // differenced in double, rounded once
+    }
+    return KBMOD_OK;
+}
+
+static bool have_device() {
+    int n = 0;
+    return cudaGetDeviceCount(&n) == cudaSuccess && n > 0;
+}
+
+struct WorkspaceLayout {
+    size_t vel_off, plan_off, enc_off, total;
+};
+
+static WorkspaceLayout workspace_layout(int N, int H, int W, int V, int K) {
+    WorkspaceLayout l;
+    size_t off = 0;
+    l.vel_off = off;
+    off = align_up(off + (size_t)V * sizeof(float2), 256);
+    l.plan_off = off;
+    off = align_up(off + staged_plan_bytes(N, V, K), 256);
+    l.enc_off = off;
+    off = align_up(off + (size_t)N * H * W * sizeof(float2), 256);
+    l.total = off;
+    return l;
+}
+}  // namespace kbmod
+
+using namespace kbmod;
+
+extern "C" {
+
+int kbmod_make_psi_phi(const float* sci, const float* var, const uint8_t* mask, const float* psf,
+                       int N, int H, int W, int P, float* psiphi, void* stream) {
+    if (!sci || !var || !psf || !psiphi) return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0) return KBMOD_ERR_SHAPE;
+    if (P <= 0 || (P % 2) == 0) return KBMOD_ERR_ARG;
+    if (P > KBMOD_MAX_PSF) return KBMOD_ERR_UNSUPPORTED;
+    if (((uintptr_t)psiphi & 7) || ((uintptr_t)sci & 3) || ((uintptr_t)var & 3)) return KBMOD_ERR_ALIGN;
+    for (size_t k = 0; k < (size_t)N * P * P; ++k)
+        if (!std::isfinite(psf[k])) return KBMOD_ERR_ARG;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    return launch_psi_phi(sci, var, mask, psf, N, H, W, P, reinterpret_cast<float2*>(psiphi),
+                          (cudaStream_t)stream);
+}
+
+size_t kbmod_search_workspace(int N, int H, int W, int V, int K) {
+    if (N <= 0 || H <= 0 || W <= 0 || V <= 0 || K <= 0) return 0;
+    return workspace_layout(N, H, W, V, K).total;
+}
+
+int kbmod_set_search_kernel(int which) {
+    if (which < 0 || which > 2) return KBMOD_ERR_ARG;
+    g_search_kernel.store(which);
+    return KBMOD_OK;
+}
+
+int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
+                 const float* vel_grid, int V, int K, int min_obs, const kbmod_result* out,
+                 void* workspace, size_t workspace_bytes, void* stream) {
+    if (!psiphi || !times || !vel_grid || !out || !workspace) return KBMOD_ERR_NULL;
+    if (!out->vel_idx || !out->n_obs || !out->psi || !out->phi || !out->nu || !out->alpha)
+        return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0 || V <= 0) return KBMOD_ERR_SHAPE;
+    if (N > KBMOD_MAX_IMAGES || K > KBMOD_MAX_K) return KBMOD_ERR_UNSUPPORTED;
+    if (K < 1 || min_obs < 1 || min_obs > N) return KBMOD_ERR_ARG;
+    if (((uintptr_t)psiphi & 15) || ((uintptr_t)workspace & 255)) return KBMOD_ERR_ALIGN;
+    if (((uintptr_t)out->vel_idx | (uintptr_t)out->n_obs | (uintptr_t)out->psi |
+         (uintptr_t)out->phi | (uintptr_t)out->nu | (uintptr_t)out->alpha) & 3)
+        return KBMOD_ERR_ALIGN;
+    for (int j = 0; j < 2 * V; ++j)
+        if (!std::isfinite(vel_grid[j])) return KBMOD_ERR_ARG;
+    DtTable dt;
+    if (int rc = make_dt(times, N, dt)) return rc;
+    const WorkspaceLayout l = workspace_layout(N, H, W, V, K);
+    if (workspace_bytes < l.total) return KBMOD_ERR_WORKSPACE;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+
+    cudaStream_t st = (cudaStream_t)stream;
+    char* ws = static_cast<char*>(workspace);
+    const float2* pp = reinterpret_cast<const float2*>(psiphi);
+    const int which = g_search_kernel.load();
+
+    if (which != 1) {
+        const int rc = launch_search_staged(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out,
+                                            ws + l.plan_off, reinterpret_cast<float2*>(ws + l.enc_off), st);
+        if (rc != KBMOD_ERR_UNSUPPORTED || which == 2) return rc;
+    }
+    float2* vel_dev = reinterpret_cast<float2*>(ws + l.vel_off);
+    if (cudaMemcpyAsync(vel_dev, vel_grid, (size_t)V * sizeof(float2), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return KBMOD_ERR_CUDA;
+    return launch_search_direct(pp, dt, N, H, W, vel_dev, V, K, min_obs, *out, st);
+}
+
+int kbmod_search_split(const float* psi, const float* phi, const double* times, int N, int H,
+                       int W, const float* vel_grid, int V, int K, int min_obs,
+                       const kbmod_result* out, void* workspace, size_t workspace_bytes,
+                       void* stream) {
+    if (!psi || !phi || !workspace) return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0 || V <= 0 || K <= 0) return KBMOD_ERR_SHAPE;
+    if ((uintptr_t)workspace & 255) return KBMOD_ERR_ALIGN;
+    const size_t need = kbmod_search_workspace(N, H, W, V, K);
+    const size_t n = (size_t)N * H * W;
+    if (workspace_bytes < need + n * sizeof(float2)) return KBMOD_ERR_WORKSPACE;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    float2* inter = reinterpret_cast<float2*>(static_cast<char*>(workspace) + need);
+    if (int rc = launch_interleave(psi, phi, n, inter, (cudaStream_t)stream)) return rc;
+    return kbmod_search(reinterpret_cast<const float*>(inter), times, N, H, W, vel_grid, V, K,
+                        min_obs, out, workspace, need, stream);
+}
+
+int kbmod_eval_trajectories(const float* psiphi, const double* times, int N, int H, int W,
+                            const int32_t* x0y0, const float* vxvy, int M, float* Psi, float* Phi,
+                            int32_t* n_obs, int32_t* ixiy, void* stream) {
+    if (!psiphi || !times || !Psi || !Phi || !n_obs) return KBMOD_ERR_NULL;
+    if (M > 0 && (!x0y0 || !vxvy)) return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0 || M < 0) return KBMOD_ERR_SHAPE;
+    if (N > KBMOD_MAX_IMAGES) return KBMOD_ERR_UNSUPPORTED;
+    if (((uintptr_t)psiphi & 7) || ((uintptr_t)vxvy & 7)) return KBMOD_ERR_ALIGN;
+    DtTable dt;
+    if (int rc = make_dt(times, N, dt)) return rc;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    return launch_eval_trajectories(reinterpret_cast<const float2*>(psiphi), dt, N, H, W, x0y0,
+                                    reinterpret_cast<const float2*>(vxvy), M, Psi, Phi, n_obs, ixiy,
+                                    (cudaStream_t)stream);
+}
+
+unsigned long long kbmod_launch_count(void) { return g_launches.load(); }
+
+const char* kbmod_status_string(int status) {
+    switch (status) {
+        case KBMOD_OK: return "ok";
+        case KBMOD_ERR_NULL: return "required pointer is NULL";
+        case KBMOD_ERR_SHAPE: return "non-positive or inconsistent dimension";
+        case KBMOD_ERR_ARG: return "argument out of range";
+        case KBMOD_ERR_ALIGN: return "pointer not aligned as documented";
+        case KBMOD_ERR_CUDA: return "CUDA error or no CUDA device";
+        case KBMOD_ERR_UNSUPPORTED: return "beyond the supported limits";
+        case KBMOD_ERR_WORKSPACE: return "workspace too small";
+    }
+    return "unknown status";
+}
+
+const char* kbmod_version(void) { return "0.1"; }
+
+}  // extern "C"

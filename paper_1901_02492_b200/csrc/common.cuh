@@ -1,0 +1,45 @@
+// common.cuh -- shared declarations of the CUDA path (internal; not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "kbmod_b200.h"
+
+namespace kbmod {
+
+// every kernel launch of the library goes through this counter (kbmod_launch_count()).
+void note_launch(int n = 1);
+
+struct DtTable {                 // dt_i = (float)(times[i] - times[0]); passed by value
+    float dt[KBMOD_MAX_IMAGES];
+};
+
+// ---- psi/phi builder (psi_phi.cu)
+int launch_psi_phi(const float* sci, const float* var, const uint8_t* mask, const float* psf_host,
+                   int N, int H, int W, int P, float2* psiphi, cudaStream_t st);
+
+// ---- direct-gather search (search_direct.cu): any shape, global loads through L1/L2
+int launch_search_direct(const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                         const float2* vel_dev, int V, int K, int min_obs,
+                         const kbmod_result& out, cudaStream_t st);
+int launch_eval_trajectories(const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                             const int32_t* x0y0, const float2* vxvy, int M, float* Psi,
+                             float* Phi, int32_t* n_obs, int32_t* ixiy, cudaStream_t st);
+int launch_interleave(const float* psi, const float* phi, size_t n, float2* out, cudaStream_t st);
+
+// ---- S3: the trajectory pixel, exactly as include/kbmod_b200.h states it
+__device__ __forceinline__ bool traj_pixel(int p0, float v, float dt, int n, int& ip) {
+    const float f = __fadd_rn(__int2float_rn(p0), __fmul_rn(v, dt));
+    const float g = floorf(__fadd_rn(f, 0.5f));
+    if (!(g >= 0.0f && g < (float)n)) return false;
+    ip = (int)g;
+    return true;
+}
+
+// ---- S5
+__device__ __forceinline__ float score_nu(float Psi, float Phi) {
+    return __fdiv_rn(Psi, __fsqrt_rn(Phi));
+}
+__device__ __forceinline__ float score_alpha(float Psi, float Phi) { return __fdiv_rn(Psi, Phi); }
+
+}  // namespace kbmod
