@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the KBMOD shift-and-stack hot path on B200.
+
+A "step" is one pass of the whole hot path (S1..S6: kbmod_make_psi_phi + kbmod_search) over one
+synthetic DECam-shaped stack.  Default workload = BASELINE.json configs[2], the configuration the
+metric is quoted on (15 x 4096 x 4096, 640 velocities, K=8, min_obs=8; 1.07e10 trajectories,
+1.61e11 trajectory-evals).  `value` = trajectory-evals/s of the whole step with inputs resident in
+HBM; `e2e` = the same through the public API from pinned HOST buffers (H2D of sci/var/mask and D2H
+of the result planes inside the timed region).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3] [--kernel 0]
+
+N > 1 (torchrun): every rank searches its own independent stack (the survey's fields/CCDs are
+independent searches) -- weak scaling, no data-path collective.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1901_02492_b200 import synth  # noqa: E402
+
+METRIC = "trajectory-evals/s"
+UNIT = "trajectory-evals/s"
+SM_COUNT = 148
+LDS_BYTES_PER_CLK_PER_SM = 128          # shared-memory crossbar (B300_MICROARCH.md "LDS/STS")
+SAMPLE_BYTES = 8                        # one float2 (psi, phi) per trajectory-eval
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d.get("hbm_gbs", 6650.0)), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+def workload(args):
+    over = {}
+    if args.rows:
+        over["H"] = args.rows
+    cfg = synth.config(args.config, **over)
+    return cfg
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (profiling recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], threading.Event()
+
+    def run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True,
+                                     text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self.stop_flag.wait(0.1)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 7
+                          for n, v in zip(names, r[3:7]) if v.lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+# ----------------------------------------------------------------------------------------------
+# reference arm / cpu baseline: the oracle as it stands, on the host cores, bounded sample
+# ----------------------------------------------------------------------------------------------
+def oracle_prepare(cfg, st):
+    """A full-height psi/phi stack for the oracle's search sample, made outside any timed region
+    by repeating a 32-row band built by the oracle (the oracle's work per evaluation does not
+    depend on the values; building all 2.5e8 pixels on the CPU would take minutes)."""
+    import oracle
+    band = min(cfg.H, 32)
+    pp_band = oracle.make_psi_phi(st.sci[:, :band], st.var[:, :band], st.mask[:, :band], st.psf)
+    reps = int(math.ceil(cfg.H / band))
+    return np.ascontiguousarray(np.tile(pp_band, (1, reps, 1, 1))[:, :cfg.H])
+
+
+def oracle_sample(cfg, st, pp_full, rows):
+    """One bounded sample of the step through the oracle as it stands: psi/phi of `rows` rows of
+    every image, then the full-grid search of `rows` start rows (full images, all velocities).
+    Returns (trajectory-evals, seconds)."""
+    import oracle
+    rows = min(rows, cfg.H)
+    y0 = cfg.H // 2 - rows // 2
+    t0 = time.perf_counter()
+    oracle.make_psi_phi(st.sci[:, y0:y0 + rows], st.var[:, y0:y0 + rows],
+                        st.mask[:, y0:y0 + rows], st.psf)
+    oracle.search(pp_full, st.times, st.vel_grid, cfg.K, cfg.min_obs, mode=oracle.MODE_F32SEQ,
+                  y_begin=y0, y_end=y0 + rows)
+    return rows * cfg.W * cfg.V * cfg.N, time.perf_counter() - t0
+
+
+def sample_text(cfg, rows):
+    return (f"{min(rows, cfg.H)} of {cfg.H} start rows per step: psi/phi of those rows of all "
+            f"{cfg.N} images + search of {min(rows, cfg.H)} x {cfg.W} start pixels x {cfg.V} "
+            f"velocities x {cfg.N} images; oracle f32seq mode, OpenMP over rows")
+
+
+def run_reference(args, cfg, st):
+    import oracle
+    oracle.build()
+    pp_full = oracle_prepare(cfg, st)
+    for _ in range(args.warmup):
+        oracle_sample(cfg, st, pp_full, max(1, args.ref_rows // 8))
+    tot_e, tot_s = 0, 0.0
+    for _ in range(args.steps):
+        e, s = oracle_sample(cfg, st, pp_full, args.ref_rows)
+        tot_e += e
+        tot_s += s
+    val = tot_e / tot_s
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "config": config_dict(cfg, args),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(),
+                         "kind": "oracle", "sample": sample_text(cfg, args.ref_rows)},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def config_dict(cfg, args):
+    return {"workload": f"BASELINE.json configs[{args.config - 1}] {cfg.name}: N={cfg.N} "
+                        f"{cfg.H}x{cfg.W} fp32, V={cfg.V} ({cfg.n_angles}x{cfg.n_speeds}), "
+                        f"K={cfg.K}, min_obs={cfg.min_obs}, seed={cfg.seed}",
+            "trajectories": cfg.trajectories, "trajectory_evals": cfg.evals,
+            "step": "kbmod_make_psi_phi + kbmod_search (S1..S6)",
+            "l2": "inputs larger than L2 (stack 2.0 GB+ vs 126 MB); no flush needed",
+            "parallelism": f"independent stacks x{args.gpus}"}
+
+
+# ----------------------------------------------------------------------------------------------
+# GPU arm
+# ----------------------------------------------------------------------------------------------
+def run_gpu(args, cfg, st, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_1901_02492_b200 import binding, build
+    build.build()
+    binding.lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    binding.set_search_kernel(args.kernel)
+    N, H, W, V, K = cfg.N, cfg.H, cfg.W, cfg.V, cfg.K
+
+    # pinned host inputs and outputs (for e2e), resident device copies (for value)
+    h_sci = torch.from_numpy(st.sci).pin_memory()
+    h_var = torch.from_numpy(st.var).pin_memory()
+    h_mask = torch.from_numpy(st.mask).pin_memory()
+    d_sci, d_var, d_mask = h_sci.to(dev), h_var.to(dev), h_mask.to(dev)
+    psiphi = torch.empty((N, H, W, 2), dtype=torch.float32, device=dev)
+    out = binding.alloc_result(H, W, K, dev)
+    ws = torch.empty(binding.search_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
+    h_out = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
+    e_sci, e_var, e_mask = torch.empty_like(d_sci), torch.empty_like(d_var), torch.empty_like(d_mask)
+
+    def step_resident():
+        binding.make_psi_phi(d_sci, d_var, d_mask, st.psf, out=psiphi)
+        binding.search(psiphi, st.times, st.vel_grid, K, cfg.min_obs, out=out, workspace=ws)
+
+    def step_e2e():
+        e_sci.copy_(h_sci, non_blocking=True)
+        e_var.copy_(h_var, non_blocking=True)
+        e_mask.copy_(h_mask, non_blocking=True)
+        binding.make_psi_phi(e_sci, e_var, e_mask, st.psf, out=psiphi)
+        binding.search(psiphi, st.times, st.vel_grid, K, cfg.min_obs, out=out, workspace=ws)
+        for k in out:
+            h_out[k].copy_(out[k], non_blocking=True)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, sampler=None):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        barrier()
+        if sampler:
+            sampler.start()
+        ev[0].record()
+        for s in range(steps):
+            fn()
+            ev[s + 1].record()
+        barrier()
+        if sampler:
+            sampler.stop_flag.set()
+        total = ev[0].elapsed_time(ev[-1])
+        if world > 1:
+            t = torch.tensor([total], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            total = float(t.item())
+        return total
+
+    for _ in range(max(3, args.warmup)):
+        step_resident()
+    sampler = ClockSampler(local_rank)
+    n0 = binding.launch_count()
+    total_ms = timed(step_resident, args.steps, sampler)
+    launches = binding.launch_count() - n0
+    clocks = sampler.summary()
+
+    # per-phase device times (same stream, CUDA events), median over the timed count
+    def phase(fn, reps):
+        ts = []
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return float(np.median(ts))
+    reps = max(3, min(args.steps, 10))
+    ms_psiphi = phase(lambda: binding.make_psi_phi(d_sci, d_var, d_mask, st.psf, out=psiphi), reps)
+    ms_search = phase(lambda: binding.search(psiphi, st.times, st.vel_grid, K, cfg.min_obs,
+                                             out=out, workspace=ws), reps)
+
+    step_e2e()
+    e2e_ms = timed(step_e2e, max(1, min(args.steps, 5)))
+    e2e_steps = max(1, min(args.steps, 5))
+
+    if rank != 0:
+        return
+    hbm_gbs, sm_max_mhz, peak_src = load_peaks()
+    evals = cfg.evals * world
+    ms_per_step = total_ms / args.steps
+    value = evals / (ms_per_step * 1e-3)
+    # roofline of the dominant kernel (the search): algorithmic shared-memory sample bytes
+    # (8 B per trajectory-eval) against the LSU peak 148 SM x 128 B/clk x max SM clock
+    lsu_peak = SM_COUNT * LDS_BYTES_PER_CLK_PER_SM * sm_max_mhz * 1e6 / 1e9       # GB/s
+    achieved = cfg.evals * SAMPLE_BYTES / (ms_search * 1e-3) / 1e9
+    hbm_bytes = N * H * W * 8 + H * W * K * 24
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": config_dict(cfg, args),
+        "trajectories_per_s": cfg.trajectories * world / (ms_per_step * 1e-3),
+        "phases_ms": {"make_psi_phi": ms_psiphi, "search": ms_search},
+        "search_only": {"trajectory_evals_per_s": cfg.evals / (ms_search * 1e-3),
+                        "trajectories_per_s": cfg.trajectories / (ms_search * 1e-3)},
+        "roofline": {"bound": "smem", "achieved": achieved, "peak": lsu_peak, "unit": "GB/s",
+                     "frac": achieved / lsu_peak, "traffic": None, "kernel": "kbmod_search",
+                     "peak_source": f"148 SM x 128 B/clk x {sm_max_mhz:.0f} MHz ({peak_src} max "
+                                    "SM clock); north_star roofline = slower of HBM and LSU",
+                     "hbm": {"compulsory_bytes": hbm_bytes, "peak": hbm_gbs,
+                             "achieved": hbm_bytes / (ms_search * 1e-3) / 1e9,
+                             "floor_ms": hbm_bytes / (hbm_gbs * 1e9) * 1e3},
+                     "lsu_floor_ms": cfg.evals * SAMPLE_BYTES / (lsu_peak * 1e9) * 1e3},
+        "clocks": clocks, "gpu_launches": int(launches),
+        "e2e": {"value": evals / (e2e_ms / e2e_steps * 1e-3), "unit": UNIT,
+                "ms_per_step": e2e_ms / e2e_steps,
+                "h2d_bytes_per_step": int(h_sci.numel() * 4 + h_var.numel() * 4 + h_mask.numel()),
+                "d2h_bytes_per_step": int(sum(v.numel() * v.element_size() for v in h_out.values()))},
+    }
+    if world == 1 and not args.no_cpu:
+        import oracle
+        oracle.build()
+        del d_sci, d_var, d_mask
+        pp_full = oracle_prepare(cfg, st)
+        oracle_sample(cfg, st, pp_full, 1)
+        e, s = oracle_sample(cfg, st, pp_full, args.ref_rows)
+        line["cpu_baseline"] = {"value": e / s, "unit": UNIT, "cores": oracle.num_threads(),
+                                "kind": "oracle", "sample": sample_text(cfg, args.ref_rows),
+                                "seconds": s}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--rows", type=int, default=0, help="override H (debug only)")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 direct, 2 staged")
+    ap.add_argument("--ref-rows", type=int, default=256, help="start rows per oracle sample")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = workload(args)
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        st = synth.make_stack(cfg)
+        run_reference(args, cfg, st)
+        return
+
+    import torch.distributed as dist
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl")
+    st = synth.make_stack(cfg, seed=cfg.seed + 1000 * rank)     # an independent stack per rank
+    run_gpu(args, cfg, st, rank, world, local_rank)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -67,9 +67,11 @@ search_direct_kernel(const float2* __restrict__ psiphi, const __grid_constant__ 
             if (nu > best_nu[KMAX - 1]) {
                 // sorted insert; strict '>' keeps the smaller index first among equal nu
                 int jj = j;
+                bool shifting = false;          // after the insert the tail shifts down as is
 #pragma unroll
                 for (int k = 0; k < KMAX; ++k) {
-                    if (nu > best_nu[k]) {
+                    if (shifting || nu > best_nu[k]) {
+                        shifting = true;
                         const float tn = best_nu[k];
                         const int tj = best_j[k];
                         best_nu[k] = nu;
