@@ -5,7 +5,7 @@
 #include <vector>
 
 #include "common.cuh"
-#include "search_staged.cuh"
+#include "search_tiled.cuh"
 
 namespace kbmod {
 static std::atomic<unsigned long long> g_launches{0};
@@ -38,7 +38,7 @@ static WorkspaceLayout workspace_layout(int N, int H, int W, int V, int K) {
     l.vel_off = off;
     off = align_up(off + (size_t)V * sizeof(float2), 256);
     l.plan_off = off;
-    off = align_up(off + staged_plan_bytes(N, V, K), 256);
+    off = align_up(off + tiled_plan_bytes(N, V, K), 256);
     l.enc_off = off;
     off = align_up(off + (size_t)N * H * W * sizeof(float2), 256);
     l.total = off;
@@ -101,14 +101,15 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
     const float2* pp = reinterpret_cast<const float2*>(psiphi);
     const int which = g_search_kernel.load();
 
-    if (which != 1) {
-        const int rc = launch_search_staged(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out,
-                                            ws + l.plan_off, reinterpret_cast<float2*>(ws + l.enc_off), st);
-        if (rc != KBMOD_ERR_UNSUPPORTED || which == 2) return rc;
-    }
     float2* vel_dev = reinterpret_cast<float2*>(ws + l.vel_off);
     if (cudaMemcpyAsync(vel_dev, vel_grid, (size_t)V * sizeof(float2), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
+    if (which != 1) {
+        const int rc = launch_search_tiled(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out,
+                                           ws + l.plan_off, vel_dev,
+                                           reinterpret_cast<float2*>(ws + l.enc_off), st);
+        if (rc != KBMOD_ERR_UNSUPPORTED || which == 2) return rc;
+    }
     return launch_search_direct(pp, dt, N, H, W, vel_dev, V, K, min_obs, *out, st);
 }
 

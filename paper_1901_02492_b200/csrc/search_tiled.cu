@@ -1,0 +1,497 @@
+// search_tiled.cu -- S3..S6, the fast path of kbmod_search (Eq.24-27).
+//
+// What makes it fast (and what it keeps exact):
+//   * S3 is hoisted to the host.  d = fl(v*dt_i) is uniform over start pixels, and
+//     ix = floor(fl(fl(x0+d)+0.5f)) equals x0 + floor(d+0.5) for EVERY integer x0 of the image
+//     whenever frac(d) is farther from 0.5 than the two roundings can move the sum (a margin of a
+//     few ulp of the largest coordinate).  The host proves that per (velocity, image) and stores
+//     the integer shift; pairs it cannot prove ("unsafe") take the literal per-lane expression on
+//     the device.  The sampled pixels are therefore identical to the definition, bit for bit.
+//   * A CTA owns a tile of start pixels and walks the velocity grid in blocks of B neighbouring
+//     velocities (host-ordered along a Hilbert curve in (vx,vy), so the B windows of an image
+//     overlap and successive blocks touch neighbouring memory).  For a proven shift the 32 lanes of a
+//     warp read 32 consecutive float2 samples at  base + offset[j][i]: one IMAD.WIDE + LDG.64 per
+//     sample, no per-lane position arithmetic and no bounds test (the host-side bounding box of a
+//     velocity's shifts decides once per (tile, velocity) whether every window is inside).
+//   * The stack is re-encoded once per call as (psi, -phi) with invalid samples = (+0,+0): one
+//     packed add.rn.f32x2 accumulates both sums (adding +0 / -0 is exact, so the result equals the
+//     in-order fp32 sum over valid observations), and the sign bit of the second word is the
+//     validity flag, counted with one LEA.HI.  3 instructions per sample.
+//   * Image 0 has dt = 0: its sample is the same for every velocity and is kept in registers.
+//   * Per-pixel top-K lives in shared memory ((nu, vel_idx) x K per pixel, lane-interleaved so it
+//     is bank-conflict free); the current K-th best is cached in registers and an approximate
+//     Psi*rsqrt(Phi) pre-test keeps the correctly rounded div/sqrt and the list update off the
+//     common path.  Psi/Phi/n_obs of the K winners are re-evaluated once at the end.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "search_tiled.cuh"
+
+namespace kbmod {
+
+namespace {
+
+constexpr int THREADS = 512;
+constexpr int SH_SKIP = 0x7FFF7FFF;       // window outside any supported image
+constexpr int SH_UNSAFE = (int)0x80008000;  // shift not proven: literal per-lane S3
+constexpr int SH_LIMIT = 32000;
+constexpr int META = 8;                   // ints of per-velocity meta data in a block record
+//   meta[0] = original velocity index (or -1: padding)
+//   meta[1] = sxlo | sxhi << 16   (int16 each)      bounding box of the proven shifts, images >= 1
+//   meta[2] = sylo | syhi << 16
+//   meta[3] = 1 if every image >= 1 has a proven, in-range shift
+//   meta[4], meta[5] = vx, vy (float bits)
+
+// record of one velocity block: off[B][N], sh[B][N], meta[B][META]
+__host__ __device__ inline size_t rec_ints(int B, int N) { return (size_t)B * N * 2 + (size_t)B * META; }
+
+int block_size_for_k(int K) { return K <= 8 ? 8 : (K <= 16 ? 16 : 32); }
+
+// ---- Hilbert index of a 16-bit quantised (x, y)
+unsigned hilbert_d(unsigned x, unsigned y) {
+    unsigned d = 0;
+    for (unsigned s = 1u << 15; s > 0; s >>= 1) {
+        const unsigned rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
+        d += s * s * ((3u * rx) ^ ry);
+        if (ry == 0) {
+            if (rx == 1) { x = 65535u - x; y = 65535u - y; }
+            std::swap(x, y);
+        }
+    }
+    return d;
+}
+
+}  // namespace
+
+size_t tiled_plan_bytes(int N, int V, int K) {
+    const int B = block_size_for_k(K);
+    const size_t nblk = ((size_t)V + B - 1) / B;
+    return nblk * rec_ints(B, N) * sizeof(int) + 256;
+}
+
+// Builds the host plan; returns the number of velocity blocks.  margin: see the header comment.
+static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, int B,
+                      std::vector<int>& plan) {
+    // processing order: Hilbert curve over the velocity plane (ties and order of equal keys: index)
+    float lox = vel[0], hix = vel[0], loy = vel[1], hiy = vel[1];
+    for (int j = 1; j < V; ++j) {
+        lox = std::min(lox, vel[2 * j]); hix = std::max(hix, vel[2 * j]);
+        loy = std::min(loy, vel[2 * j + 1]); hiy = std::max(hiy, vel[2 * j + 1]);
+    }
+    const double ext = std::max({(double)hix - lox, (double)hiy - loy, 1e-30});
+    std::vector<std::pair<unsigned, int>> key(V);
+    for (int j = 0; j < V; ++j) {
+        const unsigned qx = (unsigned)std::min(65535.0, ((double)vel[2 * j] - lox) / ext * 65535.0);
+        const unsigned qy = (unsigned)std::min(65535.0, ((double)vel[2 * j + 1] - loy) / ext * 65535.0);
+        key[j] = {hilbert_d(qx, qy), j};
+    }
+    std::sort(key.begin(), key.end());
+
+    // largest coordinate magnitude any fl(x0 + d) can reach for an in-range window
+    const double cmax = 2.0 * std::max(W, H) + 4.0;
+    const double ulp = std::ldexp(1.0, (int)std::floor(std::log2(cmax)) - 23);
+    const double margin = 4.0 * ulp;   // the two roundings move the sum by at most 1 ulp(cmax)
+
+    const int nblk = (V + B - 1) / B;
+    plan.assign((size_t)nblk * rec_ints(B, N), 0);
+    for (int blk = 0; blk < nblk; ++blk) {
+        int* off = plan.data() + (size_t)blk * rec_ints(B, N);
+        int* sh = off + (size_t)B * N;
+        int* meta = sh + (size_t)B * N;
+        for (int b = 0; b < B; ++b) {
+            const int jj = blk * B + b;
+            int* m = meta + b * META;
+            if (jj >= V) {                       // padding velocity: never scored, never sampled
+                m[0] = -1; m[3] = 0;
+                for (int i = 0; i < N; ++i) { off[b * N + i] = 0; sh[b * N + i] = SH_SKIP; }
+                continue;
+            }
+            const int j = key[jj].second;
+            const float vx = vel[2 * j], vy = vel[2 * j + 1];
+            m[0] = j;
+            std::memcpy(&m[4], &vx, 4);
+            std::memcpy(&m[5], &vy, 4);
+            int sxlo = SH_LIMIT, sxhi = -SH_LIMIT, sylo = SH_LIMIT, syhi = -SH_LIMIT, all_ok = 1;
+            for (int i = 0; i < N; ++i) {
+                // d exactly as the device would form it: one fp32 multiply (never contracted)
+                volatile float dxf = vx * dt.dt[i];
+                volatile float dyf = vy * dt.dt[i];
+                const double dx = dxf, dy = dyf;
+                int code;
+                long long o = 0;
+                if (!(std::fabs(dx) < SH_LIMIT && std::fabs(dy) < SH_LIMIT)) {
+                    code = SH_SKIP;              // farther than any supported image: no observation
+                } else {
+                    const double fx = dx - std::floor(dx), fy = dy - std::floor(dy);
+                    if (std::fabs(fx - 0.5) <= margin || std::fabs(fy - 0.5) <= margin) {
+                        code = SH_UNSAFE;
+                    } else {
+                        const int sx = (int)std::floor(dx + 0.5), sy = (int)std::floor(dy + 0.5);
+                        code = (int)(((unsigned)sy << 16) | ((unsigned)sx & 0xFFFFu));
+                        o = (long long)i * H * W + (long long)sy * W + sx;
+                        if (i >= 1) {
+                            sxlo = std::min(sxlo, sx); sxhi = std::max(sxhi, sx);
+                            sylo = std::min(sylo, sy); syhi = std::max(syhi, sy);
+                        }
+                    }
+                }
+                if (i >= 1 && (code == SH_SKIP || code == SH_UNSAFE)) all_ok = 0;
+                off[b * N + i] = (int)o;
+                sh[b * N + i] = code;
+            }
+            if (N == 1) { sxlo = sxhi = sylo = syhi = 0; }
+            m[1] = (int)(((unsigned)sxhi << 16) | ((unsigned)sxlo & 0xFFFFu));
+            m[2] = (int)(((unsigned)syhi << 16) | ((unsigned)sylo & 0xFFFFu));
+            m[3] = all_ok;
+        }
+    }
+    return nblk;
+}
+
+// ---------------------------------------------------------------------------------------------
+// device side
+// ---------------------------------------------------------------------------------------------
+
+// (psi, phi) -> (psi, -phi), invalid (psi NaN) -> (+0, +0).  Two pixels per thread (float4).
+__global__ void __launch_bounds__(256)
+encode_kernel(const float4* __restrict__ in, float4* __restrict__ out, size_t n2,
+              const float2* __restrict__ in1, float2* __restrict__ out1, size_t n) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n2; k += stride) {
+        float4 v = __ldg(in + k);
+        float4 o;
+        const bool a = (v.x == v.x), b = (v.z == v.z);
+        o.x = a ? v.x : 0.0f;
+        o.y = a ? -v.y : 0.0f;
+        o.z = b ? v.z : 0.0f;
+        o.w = b ? -v.w : 0.0f;
+        out[k] = o;
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {   // odd tail pixel
+        const float2 v = in1[n - 1];
+        const bool a = (v.x == v.x);
+        out1[n - 1] = make_float2(a ? v.x : 0.0f, a ? -v.y : 0.0f);
+    }
+}
+
+typedef unsigned long long u64;
+
+__device__ __forceinline__ void acc_add(u64& a, u64 s) {      // (Psi, -Phi) += (psi, -phi), RN each
+    asm("add.rn.f32x2 %0, %0, %1;" : "+l"(a) : "l"(s));
+}
+__device__ __forceinline__ u64 ld_sample(const u64* p) { return __ldg(p); }
+
+struct TiledParams {
+    const float2* psiphi;     // original stack (final re-evaluation of the winners)
+    const u64* enc;           // encoded stack
+    const int* plan;          // nblk records
+    const float2* vel;        // caller's velocity table (device copy)
+    int nblk, N, H, W, K, min_obs;
+    int tiles_x, tiles_y, group_w;
+    kbmod_result out;
+    DtTable dt;
+};
+
+// RX x RY pixels per thread: x = tile_x + (warp % WX) * 32 * RX + rx * 32 + lane,
+//                            y = tile_y + (warp / WX) * RY + ry
+template <int RX, int RY, int WX, int B, int KMAX>
+struct TileGeom {
+    static constexpr int R = RX * RY;
+    static constexpr int WARPS = THREADS / 32;
+    static constexpr int TW = 32 * RX * WX;
+    static constexpr int TH = RY * (WARPS / WX);
+    static constexpr int PX = THREADS * R;
+    static size_t smem_bytes(int N) {
+        return (size_t)PX * KMAX * 8 + rec_ints(B, N) * sizeof(int);
+    }
+};
+
+template <int RX, int RY, int WX, int B, int KMAX>
+__global__ void __launch_bounds__(THREADS, 1)
+search_tiled_kernel(const __grid_constant__ TiledParams prm) {
+    using G = TileGeom<RX, RY, WX, B, KMAX>;
+    constexpr int R = G::R;
+    constexpr int PX = G::PX;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* l_nu = reinterpret_cast<float*>(smem_raw);            // [KMAX][PX]
+    int* l_idx = reinterpret_cast<int*>(l_nu + (size_t)KMAX * PX);   // [KMAX][PX]
+    int* rec = l_idx + (size_t)KMAX * PX;                         // off[B][N], sh[B][N], meta[B][META]
+
+    const int N = prm.N, H = prm.H, W = prm.W, K = prm.K;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    // tile of this CTA: groups of group_w tile columns, row-major inside a group, so that the CTAs
+    // running at the same time cover a compact region (their windows then share L2 lines)
+    int tx, ty;
+    {
+        const int per_group = prm.group_w * prm.tiles_y;
+        const int g = blockIdx.x / per_group, rem = blockIdx.x - g * per_group;
+        const int gw = min(prm.group_w, prm.tiles_x - g * prm.group_w);
+        ty = rem / gw;
+        tx = g * prm.group_w + (rem - ty * gw);
+    }
+    const int tile_x = tx * G::TW, tile_y = ty * G::TH;
+    const int x_first = tile_x + (warp % WX) * 32 * RX + lane;
+    const int y_first = tile_y + (warp / WX) * RY;
+    const bool ragged = (tile_x + G::TW > W) || (tile_y + G::TH > H);
+    // tile extent that holds real pixels (for window classification)
+    const int tile_x1 = min(tile_x + G::TW, W) - 1, tile_y1 = min(tile_y + G::TH, H) - 1;
+
+    const u64* basep[RY];
+#pragma unroll
+    for (int ry = 0; ry < RY; ++ry)
+        basep[ry] = prm.enc + (size_t)min(y_first + ry, H - 1) * W + min(x_first, W - 1);
+
+    // per-pixel list state: nu of the worst entry (the K-th best once the list is full)
+    float w_nu[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        w_nu[r] = -INFINITY;
+        for (int e = 0; e < K; ++e) {
+            l_nu[e * PX + r * THREADS + tid] = -INFINITY;
+            l_idx[e * PX + r * THREADS + tid] = 0x7FFFFFFF;
+        }
+    }
+
+    const int rec_n = (int)rec_ints(B, N);
+    int* r_off = rec;
+    int* r_sh = rec + B * N;
+    int* r_meta = rec + 2 * B * N;
+
+    for (int blk = 0; blk < prm.nblk; ++blk) {
+        __syncthreads();
+        {
+            const int* src = prm.plan + (size_t)blk * rec_n;
+            for (int k = tid; k < rec_n; k += THREADS) rec[k] = __ldg(src + k);
+        }
+        __syncthreads();
+
+        u64 acc[B][R];
+        unsigned cnt[B][R];
+        unsigned fast = 0;          // bit b: every window of velocity b is inside the image
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+#pragma unroll
+            for (int ry = 0; ry < RY; ++ry)
+#pragma unroll
+                for (int rx = 0; rx < RX; ++rx) {
+                    // image 0 has dt = 0: shift (0,0) for every velocity
+                    const bool inimg = (x_first + 32 * rx < W) && (y_first + ry < H);
+                    const u64 s0 = inimg ? ld_sample(basep[ry] + 32 * rx) : 0ull;
+                    acc[b][ry * RX + rx] = s0;
+                    cnt[b][ry * RX + rx] = (unsigned)(s0 >> 63);
+                }
+            const int bx = r_meta[b * META + 1], by = r_meta[b * META + 2];
+            const int sxlo = (short)(bx & 0xFFFF), sxhi = bx >> 16;
+            const int sylo = (short)(by & 0xFFFF), syhi = by >> 16;
+            const bool ok = r_meta[b * META + 3] && !ragged && tile_x + sxlo >= 0 &&
+                            tile_x1 + sxhi < W && tile_y + sylo >= 0 && tile_y1 + syhi < H;
+            fast |= ok ? (1u << b) : 0u;
+        }
+
+        for (int i = 1; i < N; ++i) {
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                if (fast & (1u << b)) {
+                    const int o = r_off[b * N + i];
+#pragma unroll
+                    for (int ry = 0; ry < RY; ++ry) {
+                        const u64* p = basep[ry] + o;
+#pragma unroll
+                        for (int rx = 0; rx < RX; ++rx) {
+                            const u64 s = ld_sample(p + 32 * rx);
+                            acc_add(acc[b][ry * RX + rx], s);
+                            cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
+                        }
+                    }
+                } else {
+                    const int code = r_sh[b * N + i];
+                    if (code == SH_SKIP) continue;
+                    const u64* img = prm.enc + (size_t)i * H * W;
+                    if (code != SH_UNSAFE) {
+                        const int sx = (short)(code & 0xFFFF), sy = code >> 16;
+                        // whole window outside: nothing to add (uniform over the CTA)
+                        if (tile_x1 + sx < 0 || tile_x + sx >= W || tile_y1 + sy < 0 || tile_y + sy >= H)
+                            continue;
+#pragma unroll
+                        for (int ry = 0; ry < RY; ++ry) {
+                            const int y = y_first + ry + sy;
+                            const bool yin = (y_first + ry < H) && y >= 0 && y < H;
+#pragma unroll
+                            for (int rx = 0; rx < RX; ++rx) {
+                                const int x = x_first + 32 * rx + sx;
+                                const bool in = yin && (x_first + 32 * rx < W) && x >= 0 && x < W;
+                                const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
+                                acc_add(acc[b][ry * RX + rx], s);
+                                cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
+                            }
+                        }
+                    } else {
+                        const float vx = __int_as_float(r_meta[b * META + 4]);
+                        const float vy = __int_as_float(r_meta[b * META + 5]);
+                        const float dti = prm.dt.dt[i];
+#pragma unroll
+                        for (int ry = 0; ry < RY; ++ry) {
+                            int y = 0;
+                            const bool yin = traj_pixel(y_first + ry, vy, dti, H, y) && (y_first + ry < H);
+#pragma unroll
+                            for (int rx = 0; rx < RX; ++rx) {
+                                int x = 0;
+                                const bool in = traj_pixel(x_first + 32 * rx, vx, dti, W, x) && yin &&
+                                                (x_first + 32 * rx < W);
+                                const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
+                                acc_add(acc[b][ry * RX + rx], s);
+                                cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+
+        // S5 + S6 for the B x R trajectories of this block
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int j = r_meta[b * META + 0];
+            if (j < 0) continue;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const float Psi = __uint_as_float((unsigned)acc[b][r]);
+                const float Phi = 0.0f - __uint_as_float((unsigned)(acc[b][r] >> 32));
+                if ((int)cnt[b][r] >= prm.min_obs && Phi > 0.0f) {
+                    const float approx = Psi * rsqrtf(Phi);
+                    const float lo = fmaf(-fabsf(w_nu[r]), 4e-6f, w_nu[r]);   // -inf stays -inf
+                    if (!(approx < lo)) {
+                        const float nu = score_nu(Psi, Phi);
+                        const int p = r * THREADS + tid;
+                        // worst (smallest nu, ties -> larger index) and second-worst entries
+                        float wn = INFINITY, vn = INFINITY;
+                        int wj = -1, vj = -1, ws = 0;
+                        for (int e = 0; e < K; ++e) {
+                            const float ne = l_nu[e * PX + p];
+                            const int je = l_idx[e * PX + p];
+                            if (ne < wn || (ne == wn && je > wj)) {
+                                vn = wn; vj = wj;
+                                wn = ne; wj = je; ws = e;
+                            } else if (ne < vn || (ne == vn && je > vj)) {
+                                vn = ne; vj = je;
+                            }
+                        }
+                        if (nu > wn || (nu == wn && j < wj)) {
+                            l_nu[ws * PX + p] = nu;
+                            l_idx[ws * PX + p] = j;
+                            // the new worst is the old second-worst or the candidate itself
+                            w_nu[r] = (nu < vn || (nu == vn && j > vj)) ? nu : vn;
+                        }
+                    }
+                }
+            }
+        }
+    }
+
+    // ---- output: K entries per pixel, best first; winners re-evaluated with the literal S3+S4
+#pragma unroll 1
+    for (int r = 0; r < R; ++r) {
+        const int rx = r % RX, ry = r / RX;
+        const int x0 = x_first + 32 * rx, y0 = y_first + ry;
+        if (x0 >= W || y0 >= H) continue;
+        const int p = r * THREADS + tid;
+        const size_t obase = ((size_t)y0 * W + x0) * K;
+        for (int k = 0; k < K; ++k) {
+            float bn = -INFINITY;
+            int bj = 0x7FFFFFFF, bs = -1;
+            for (int e = 0; e < K; ++e) {
+                const float ne = l_nu[e * PX + p];
+                const int je = l_idx[e * PX + p];
+                if (je != 0x7FFFFFFF && (bs < 0 || ne > bn || (ne == bn && je < bj))) { bn = ne; bj = je; bs = e; }
+            }
+            if (bs >= 0) {
+                l_idx[bs * PX + p] = 0x7FFFFFFF;
+                // literal evaluation (bit-identical sums: same samples, same order)
+                float Psi = 0.0f, Phi = 0.0f;
+                int n = 0;
+                const float2 v = __ldg(prm.vel + bj);
+                for (int i = 0; i < N; ++i) {
+                    int ix, iy;
+                    if (traj_pixel(x0, v.x, prm.dt.dt[i], W, ix) && traj_pixel(y0, v.y, prm.dt.dt[i], H, iy)) {
+                        const float2 s = __ldg(prm.psiphi + ((size_t)i * H + iy) * W + ix);
+                        if (s.x == s.x) { Psi = __fadd_rn(Psi, s.x); Phi = __fadd_rn(Phi, s.y); ++n; }
+                    }
+                }
+                prm.out.vel_idx[obase + k] = bj;
+                prm.out.n_obs[obase + k] = n;
+                prm.out.psi[obase + k] = Psi;
+                prm.out.phi[obase + k] = Phi;
+                prm.out.nu[obase + k] = score_nu(Psi, Phi);
+                prm.out.alpha[obase + k] = score_alpha(Psi, Phi);
+            } else {
+                prm.out.vel_idx[obase + k] = -1;
+                prm.out.n_obs[obase + k] = 0;
+                prm.out.psi[obase + k] = 0.0f;
+                prm.out.phi[obase + k] = 0.0f;
+                prm.out.nu[obase + k] = -INFINITY;
+                prm.out.alpha[obase + k] = 0.0f;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// launch
+// ---------------------------------------------------------------------------------------------
+template <int RX, int RY, int WX, int B, int KMAX>
+static int launch_variant(TiledParams& prm, cudaStream_t st) {
+    using G = TileGeom<RX, RY, WX, B, KMAX>;
+    const size_t smem = G::smem_bytes(prm.N);
+    if (smem > 227 * 1024) return KBMOD_ERR_UNSUPPORTED;
+    auto kern = search_tiled_kernel<RX, RY, WX, B, KMAX>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess)
+            return KBMOD_ERR_CUDA;
+        attr_set = true;
+    }
+    prm.tiles_x = (prm.W + G::TW - 1) / G::TW;
+    prm.tiles_y = (prm.H + G::TH - 1) / G::TH;
+    prm.group_w = std::max(1, 512 / G::TW);
+    const long long tiles = (long long)prm.tiles_x * prm.tiles_y;
+    if (tiles > 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
+    kern<<<(unsigned)tiles, THREADS, smem, st>>>(prm);
+    note_launch();
+    return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
+}
+
+int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                        const float* vel_host, int V, int K, int min_obs, const kbmod_result& out,
+                        void* plan_dev, const float2* vel_dev, float2* enc_dev, cudaStream_t st) {
+    // limits of the int16 shift encoding and of the int32 element offsets
+    if (W > 30000 || H > 30000) return KBMOD_ERR_UNSUPPORTED;
+    if ((long long)(N + 1) * H * W + (long long)SH_LIMIT * (W + 1) >= 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
+    const int B = block_size_for_k(K);
+    std::vector<int> plan;
+    const int nblk = build_plan(dt, N, H, W, vel_host, V, B, plan);
+    if (cudaMemcpyAsync(plan_dev, plan.data(), plan.size() * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return KBMOD_ERR_CUDA;
+
+    const size_t n = (size_t)N * H * W;
+    encode_kernel<<<148 * 8, 256, 0, st>>>(reinterpret_cast<const float4*>(psiphi),
+                                          reinterpret_cast<float4*>(enc_dev), n / 2, psiphi, enc_dev, n);
+    note_launch();
+    if (cudaGetLastError() != cudaSuccess) return KBMOD_ERR_CUDA;
+
+    TiledParams prm;
+    prm.psiphi = psiphi;
+    prm.enc = reinterpret_cast<const u64*>(enc_dev);
+    prm.plan = static_cast<const int*>(plan_dev);
+    prm.vel = vel_dev;
+    prm.nblk = nblk; prm.N = N; prm.H = H; prm.W = W; prm.K = K; prm.min_obs = min_obs;
+    prm.out = out;
+    prm.dt = dt;
+    if (K <= 8) return launch_variant<2, 2, 1, 8, 8>(prm, st);      // tile 64 x 32
+    if (K <= 16) return launch_variant<2, 1, 1, 16, 16>(prm, st);   // tile 64 x 16
+    return launch_variant<1, 1, 1, 32, 32>(prm, st);                // tile 32 x 16
+}
+
+}  // namespace kbmod
