@@ -130,9 +130,11 @@ int kbmod_eval_trajectories(const float* psiphi, const double* times, int N, int
                             float* Psi, float* Phi, int32_t* n_obs, int32_t* ixiy,
                             void* stream);
 
-/* Selects the search kernel: 0 = automatic (default), 1 = direct-gather kernel (global loads,
- * any shape), 2 = shared-memory staged kernel (KBMOD_ERR_UNSUPPORTED from kbmod_search if the
- * shape does not fit it).  Process-wide; for tests and benchmarks. */
+/* Selects the search kernel: 0 = automatic (default: the tiled kernel where the shape fits, else
+ * the direct-gather kernel), 1 = direct-gather kernel (global loads, any shape), 2 = tiled kernel
+ * (host-proven integer shifts, global loads through L1), 3 = TMA-staged shared-memory kernel.
+ * With 2 or 3 kbmod_search returns KBMOD_ERR_UNSUPPORTED if the shape does not fit that kernel.
+ * Process-wide; for tests and benchmarks. */
 int kbmod_set_search_kernel(int which);
 
 /* Number of kernel launches issued by this library since load (for benchmark accounting). */

@@ -1,10 +1,12 @@
 // api.cu -- the C ABI of include/kbmod_b200.h: argument checks, host-side tables, dispatch.
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstring>
 #include <vector>
 
 #include "common.cuh"
+#include "search_staged.cuh"
 #include "search_tiled.cuh"
 
 namespace kbmod {
@@ -38,9 +40,9 @@ static WorkspaceLayout workspace_layout(int N, int H, int W, int V, int K) {
     l.vel_off = off;
     off = align_up(off + (size_t)V * sizeof(float2), 256);
     l.plan_off = off;
-    off = align_up(off + tiled_plan_bytes(N, V, K), 256);
+    off = align_up(off + std::max(staged_plan_bytes(N, V), tiled_plan_bytes(N, V, K)), 256);
     l.enc_off = off;
-    off = align_up(off + (size_t)N * H * W * sizeof(float2), 256);
+    off = align_up(off + staged_enc_bytes(N, H, W), 256);
     l.total = off;
     return l;
 }
@@ -70,7 +72,7 @@ size_t kbmod_search_workspace(int N, int H, int W, int V, int K) {
 }
 
 int kbmod_set_search_kernel(int which) {
-    if (which < 0 || which > 2) return KBMOD_ERR_ARG;
+    if (which < 0 || which > 3) return KBMOD_ERR_ARG;
     g_search_kernel.store(which);
     return KBMOD_OK;
 }
@@ -104,6 +106,9 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
     float2* vel_dev = reinterpret_cast<float2*>(ws + l.vel_off);
     if (cudaMemcpyAsync(vel_dev, vel_grid, (size_t)V * sizeof(float2), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
+    if (which == 3)      // TMA-staged kernel: opt-in until it has been validated on hardware
+        return launch_search_staged(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out, ws + l.plan_off, vel_dev,
+                                    reinterpret_cast<float2*>(ws + l.enc_off), st);
     if (which != 1) {
         const int rc = launch_search_tiled(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out,
                                            ws + l.plan_off, vel_dev,

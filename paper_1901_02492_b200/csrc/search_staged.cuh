@@ -1,0 +1,21 @@
+// search_staged.cuh -- interface of the TMA-staged search kernel (search_staged.cu).
+#pragma once
+#include "common.cuh"
+
+namespace kbmod {
+
+// bytes of device scratch the staged kernel needs besides the encoded stack: the entry stream
+// (upper bound for these sizes)
+size_t staged_plan_bytes(int N, int V);
+// bytes of the encoded stack (row pitch padded to an even number of samples)
+size_t staged_enc_bytes(int N, int H, int W);
+
+// S3..S6 with host-planned integer shifts and TMA-staged shared-memory windows.  Returns
+// KBMOD_ERR_UNSUPPORTED when the shape does not fit this kernel (the caller then uses the
+// direct-gather kernel).  plan_dev / enc_dev are carved from the caller's workspace
+// (staged_plan_bytes() / staged_enc_bytes()); vel_dev is the device copy of the velocity table.
+int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                         const float* vel_host, int V, int K, int min_obs, const kbmod_result& out,
+                         void* plan_dev, const float2* vel_dev, float2* enc_dev, cudaStream_t st);
+
+}  // namespace kbmod
