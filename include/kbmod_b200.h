@@ -137,6 +137,22 @@ int kbmod_eval_trajectories(const float* psiphi, const double* times, int N, int
  * Process-wide; for tests and benchmarks. */
 int kbmod_set_search_kernel(int which);
 
+/*
+ * Test hook (host only, no CUDA call): the plan the TMA-staged kernel would execute for these
+ * inputs, so that its host logic -- the proof that one integer shift per (velocity, image)
+ * reproduces S3 for every start pixel, the grouping of shifted windows into shared-memory boxes,
+ * the per-member offsets -- can be checked against the oracle without a GPU.
+ *   times, vel_grid : HOST, as for kbmod_search
+ *   stream  : HOST out, nent entries of info[1] int32 each (layout: csrc/search_staged.cu)
+ *   shapes  : HOST out, [nshapes][2] = (box width, box height) in samples, index = tensor-map id
+ *   info    : HOST out [8] = nent, ints per entry, nshapes, tile width, tile height, velocities
+ *             per block, samples per slot, header bytes
+ * Returns KBMOD_ERR_WORKSPACE (with info filled) if stream_ints / max_shapes are too small.
+ */
+int kbmod_debug_staged_plan(const double* times, int N, int H, int W, const float* vel_grid, int V,
+                            int32_t* stream, size_t stream_ints, int32_t* shapes, int max_shapes,
+                            int32_t* info);
+
 /* Number of kernel launches issued by this library since load (for benchmark accounting). */
 unsigned long long kbmod_launch_count(void);
 

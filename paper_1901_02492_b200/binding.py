@@ -19,7 +19,7 @@ _lib: Optional[ctypes.CDLL] = None
 
 EXPORTS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_workspace", "kbmod_search_split",
            "kbmod_eval_trajectories", "kbmod_set_search_kernel", "kbmod_launch_count",
-           "kbmod_status_string", "kbmod_version")
+           "kbmod_status_string", "kbmod_version", "kbmod_debug_staged_plan")
 
 
 class KbmodError(RuntimeError):
@@ -43,7 +43,8 @@ def lib() -> ctypes.CDLL:
         L.kbmod_status_string.restype = ctypes.c_char_p
         L.kbmod_version.restype = ctypes.c_char_p
         for n in ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_split",
-                  "kbmod_eval_trajectories", "kbmod_set_search_kernel"):
+                  "kbmod_eval_trajectories", "kbmod_set_search_kernel",
+                  "kbmod_debug_staged_plan"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -82,6 +83,29 @@ def launch_count() -> int:
 
 def set_search_kernel(which: int) -> None:
     _check(lib().kbmod_set_search_kernel(int(which)), "kbmod_set_search_kernel")
+
+
+def debug_staged_plan(times, N: int, H: int, W: int, vel_grid):
+    """kbmod_debug_staged_plan (host only): returns (stream [nent, ints_per_entry] int32,
+    shapes [nshapes, 2] int32, info dict)."""
+    t = _host(times, np.float64)
+    v = _host(vel_grid, np.float32).reshape(-1, 2)
+    V = v.shape[0]
+    B_guess = 8
+    cap = (V // B_guess + 2) * (max(N - 1, 0) * B_guess + 1) * 128
+    stream = np.zeros(cap, np.int32)
+    shapes = np.zeros((4096, 2), np.int32)
+    info = np.zeros(8, np.int32)
+    rc = lib().kbmod_debug_staged_plan(t.ctypes.data_as(ctypes.c_void_p), N, H, W,
+                                       v.ctypes.data_as(ctypes.c_void_p), V,
+                                       stream.ctypes.data_as(ctypes.c_void_p), ctypes.c_size_t(cap),
+                                       shapes.ctypes.data_as(ctypes.c_void_p), 4096,
+                                       info.ctypes.data_as(ctypes.c_void_p))
+    _check(rc, "kbmod_debug_staged_plan")
+    keys = ("nent", "hdr_ints", "nshapes", "TW", "TH", "B", "CAP", "HDR_BYTES")
+    d = {k: int(x) for k, x in zip(keys, info)}
+    return stream[:d["nent"] * d["hdr_ints"]].reshape(d["nent"], d["hdr_ints"]).copy(), \
+        shapes[:d["nshapes"]].copy(), d
 
 
 def search_workspace(N: int, H: int, W: int, V: int, K: int) -> int:

@@ -151,6 +151,19 @@ int kbmod_eval_trajectories(const float* psiphi, const double* times, int N, int
                                     (cudaStream_t)stream);
 }
 
+int kbmod_debug_staged_plan(const double* times, int N, int H, int W, const float* vel_grid, int V,
+                            int32_t* stream, size_t stream_ints, int32_t* shapes, int max_shapes,
+                            int32_t* info) {
+    if (!times || !vel_grid || !stream || !shapes || !info) return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0 || V <= 0 || max_shapes < 0) return KBMOD_ERR_SHAPE;
+    if (N > KBMOD_MAX_IMAGES) return KBMOD_ERR_UNSUPPORTED;
+    for (int j = 0; j < 2 * V; ++j)
+        if (!std::isfinite(vel_grid[j])) return KBMOD_ERR_ARG;
+    DtTable dt;
+    if (int rc = make_dt(times, N, dt)) return rc;
+    return staged_plan_debug(dt, N, H, W, vel_grid, V, stream, stream_ints, shapes, max_shapes, info);
+}
+
 unsigned long long kbmod_launch_count(void) { return g_launches.load(); }
 
 const char* kbmod_status_string(int status) {

@@ -277,6 +277,23 @@ size_t staged_plan_bytes(int N, int V) {
 }
 size_t staged_enc_bytes(int N, int H, int W) { return (size_t)N * H * ((W + 1) & ~1) * sizeof(float2); }
 
+int staged_plan_debug(const DtTable& dt, int N, int H, int W, const float* vel_host, int V,
+                      int32_t* stream, size_t stream_ints, int32_t* shapes, int max_shapes, int32_t* info) {
+    if (W > SH_LIMIT || H > SH_LIMIT || V >= (1 << 24)) return KBMOD_ERR_UNSUPPORTED;
+    StagedPlan plan;
+    if (!build_plan(dt, N, H, W, vel_host, V, plan)) return KBMOD_ERR_UNSUPPORTED;
+    info[0] = plan.nent; info[1] = HDR_INTS; info[2] = (int)plan.shapes.size(); info[3] = TW;
+    info[4] = TH; info[5] = B; info[6] = CAP; info[7] = HDR_BYTES;
+    if (plan.stream.size() * sizeof(int) > staged_plan_bytes(N, V)) return KBMOD_ERR_UNSUPPORTED;
+    if (plan.stream.size() > stream_ints || (int)plan.shapes.size() > max_shapes) return KBMOD_ERR_WORKSPACE;
+    std::memcpy(stream, plan.stream.data(), plan.stream.size() * sizeof(int));
+    for (size_t m = 0; m < plan.shapes.size(); ++m) {
+        shapes[2 * m] = plan.shapes[m].first;
+        shapes[2 * m + 1] = plan.shapes[m].second;
+    }
+    return KBMOD_OK;
+}
+
 // ---------------------------------------------------------------------------------------------
 // device side
 // ---------------------------------------------------------------------------------------------

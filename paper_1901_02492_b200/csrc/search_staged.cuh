@@ -18,4 +18,9 @@ int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, 
                          const float* vel_host, int V, int K, int min_obs, const kbmod_result& out,
                          void* plan_dev, const float2* vel_dev, float2* enc_dev, cudaStream_t st);
 
+// Host-only: builds the entry stream for these inputs (test hook behind kbmod_debug_staged_plan).
+// info[0..7] = nent, HDR_INTS, nshapes, TW, TH, B, CAP (samples per slot), HDR_BYTES.
+int staged_plan_debug(const DtTable& dt, int N, int H, int W, const float* vel_host, int V,
+                      int32_t* stream, size_t stream_ints, int32_t* shapes, int max_shapes, int32_t* info);
+
 }  // namespace kbmod
