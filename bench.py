@@ -304,7 +304,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--rows", type=int, default=0, help="override H (debug only)")
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 direct, 2 staged")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto (tiled), 1 direct, 2 tiled, 3 TMA-staged")
     ap.add_argument("--ref-rows", type=int, default=256, help="start rows per oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()

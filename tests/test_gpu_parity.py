@@ -7,6 +7,7 @@ Bars (BASELINE.json north_star):
                    when |nu| < 1) of its f64 mode, top-K sets equal up to near-tie swaps.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -16,7 +17,10 @@ from paper_1901_02492_b200 import synth
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [1, 0]          # 1 = direct gather, 0 = automatic (staged where the shape fits)
+# 1 = direct gather, 0 = automatic (the tiled kernel where the shape fits), 3 = TMA-staged kernel.
+# The staged kernel has not yet been validated on hardware: it is only
+# exercised when KBMOD_TEST_STAGED=1, so that an untested kernel cannot take the suite down.
+KERNELS = [1, 0] + ([3] if os.environ.get("KBMOD_TEST_STAGED") == "1" else [])
 
 
 @pytest.fixture(scope="module")
