@@ -28,13 +28,17 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_1901_02492_b200 import synth  # noqa: E402
+from paper_1901_02492_b200 import shard, synth  # noqa: E402
 
 METRIC = "trajectory-evals/s"
 UNIT = "trajectory-evals/s"
 SM_COUNT = 148
 LDS_BYTES_PER_CLK_PER_SM = 128          # shared-memory crossbar (B300_MICROARCH.md "LDS/STS")
 SAMPLE_BYTES = 8                        # one float2 (psi, phi) per trajectory-eval
+# dram__bytes_read.sum + dram__bytes_write.sum of the search kernel, one launch at config 3, from
+# the committed `ncu --set full` captures (profiles/r01_v1_direct.md, profiles/r01_v2_tiled.md);
+# keyed by the kernel kbmod_set_search_kernel selects (0 = automatic = the tiled kernel).
+NCU_DRAM_BYTES_CONFIG3 = {1: 666.6e9 + 3.67e9, 0: 218.9e9 + 3.23e9, 2: 218.9e9 + 3.23e9}
 
 
 def load_peaks():
@@ -214,12 +218,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
         barrier()
         if sampler:
             sampler.stop_flag.set()
-        total = ev[0].elapsed_time(ev[-1])
-        if world > 1:
-            t = torch.tensor([total], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            total = float(t.item())
-        return total
+        return shard.max_over_ranks(ev[0].elapsed_time(ev[-1]), dev)
 
     for _ in range(max(3, args.warmup)):
         step_resident()
@@ -270,7 +269,11 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
         "search_only": {"trajectory_evals_per_s": cfg.evals / (ms_search * 1e-3),
                         "trajectories_per_s": cfg.trajectories / (ms_search * 1e-3)},
         "roofline": {"bound": "smem", "achieved": achieved, "peak": lsu_peak, "unit": "GB/s",
-                     "frac": achieved / lsu_peak, "traffic": None, "kernel": "kbmod_search",
+                     "frac": achieved / lsu_peak,
+                     "traffic": (NCU_DRAM_BYTES_CONFIG3.get(args.kernel)
+                                 if args.config == 3 and not args.rows else None),
+                     "traffic_source": "profiles/ (ncu --set full of an earlier run of this kernel)",
+                     "kernel": "kbmod_search",
                      "peak_source": f"148 SM x 128 B/clk x {sm_max_mhz:.0f} MHz ({peak_src} max "
                                     "SM clock); north_star roofline = slower of HBM and LSU",
                      "hbm": {"compulsory_bytes": hbm_bytes, "peak": hbm_gbs,
@@ -325,7 +328,7 @@ def main():
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl")
-    st = synth.make_stack(cfg, seed=cfg.seed + 1000 * rank)     # an independent stack per rank
+    st = synth.make_stack(cfg, seed=shard.rank_seed(cfg.seed, rank))     # an independent stack per rank
     run_gpu(args, cfg, st, rank, world, local_rank)
     if world > 1:
         dist.destroy_process_group()

@@ -1,0 +1,75 @@
+"""Multi-GPU plumbing of the search.  One process per GPU.
+
+The path has no exchange step ("each evaluation ... is entirely independent"): ranks
+either search independent stacks (what bench.py --gpus N times) or disjoint bands of start rows of
+one replicated stack.  The only collectives are the timing barrier / MAX reduction and, for
+bands, the concatenation of the result planes.  Works with any torch.distributed backend (NCCL on
+GPUs, gloo in the CPU tests); every function degrades to the single-process case.
+"""
+from __future__ import annotations
+
+from typing import Dict, List, Tuple
+
+import torch
+import torch.distributed as dist
+
+
+def world() -> Tuple[int, int]:
+    """(rank, world_size); (0, 1) when torch.distributed is not initialised."""
+    if dist.is_available() and dist.is_initialized():
+        return dist.get_rank(), dist.get_world_size()
+    return 0, 1
+
+
+def rank_seed(seed: int, rank: int) -> int:
+    """Seed of the independent synthetic stack a rank searches in the weak-scaling benchmark."""
+    return int(seed) + 1000 * int(rank)
+
+
+def row_bands(H: int, world_size: int) -> List[Tuple[int, int]]:
+    """Balanced contiguous bands [y0, y1) of start rows, one per rank (empty if H < world_size)."""
+    base, extra = divmod(int(H), int(world_size))
+    out, y = [], 0
+    for r in range(world_size):
+        h = base + (1 if r < extra else 0)
+        out.append((y, y + h))
+        y += h
+    return out
+
+
+def max_over_ranks(value: float, device=None) -> float:
+    """Device time of a step = the slowest rank's (MAX all-reduce); identity for one process."""
+    _, n = world()
+    if n == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def total_over_ranks(value: float, device=None) -> float:
+    """Units processed by the whole job (SUM all-reduce)."""
+    _, n = world()
+    if n == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def gather_bands(band: Dict[str, torch.Tensor], H: int) -> Dict[str, torch.Tensor]:
+    """Concatenates per-rank result planes [rows_r, W, K] of row_bands(H, world) into [H, W, K] on
+    every rank (all_gather of padded bands; no reduction: bands are disjoint)."""
+    rank, n = world()
+    if n == 1:
+        return band
+    bands = row_bands(H, n)
+    hmax = max(y1 - y0 for y0, y1 in bands)
+    out = {}
+    for k, t in band.items():
+        pad = torch.zeros((hmax,) + tuple(t.shape[1:]), dtype=t.dtype, device=t.device)
+        pad[: t.shape[0]] = t
+        parts = [torch.empty_like(pad) for _ in range(n)]
+        dist.all_gather(parts, pad)
+        out[k] = torch.cat([p[: y1 - y0] for p, (y0, y1) in zip(parts, bands)], 0)
+    return out
