@@ -222,6 +222,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
 
     for _ in range(max(3, args.warmup)):
         step_resident()
+    binding.search_status(ws)               # raises if a kernel gave up (never times a broken run)
     sampler = ClockSampler(local_rank)
     n0 = binding.launch_count()
     total_ms = timed(step_resident, args.steps, sampler)
@@ -244,6 +245,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     ms_search = phase(lambda: binding.search(psiphi, st.times, st.vel_grid, K, cfg.min_obs,
                                              out=out, workspace=ws), reps)
 
+    binding.search_status(ws)
     step_e2e()
     e2e_ms = timed(step_e2e, max(1, min(args.steps, 5)))
     e2e_steps = max(1, min(args.steps, 5))

@@ -37,7 +37,8 @@ typedef enum {
     KBMOD_ERR_ALIGN = -4,       /* pointer not aligned as documented */
     KBMOD_ERR_CUDA = -5,        /* CUDA runtime error at launch / no device */
     KBMOD_ERR_UNSUPPORTED = -6, /* beyond the supported limits (P > 31, N > 64, K > 32) */
-    KBMOD_ERR_WORKSPACE = -7    /* workspace smaller than kbmod_search_workspace() */
+    KBMOD_ERR_WORKSPACE = -7,   /* workspace smaller than kbmod_search_workspace() */
+    KBMOD_ERR_TIMEOUT = -8      /* a kernel gave up waiting on its own pipeline (kbmod_search_status) */
 } kbmod_status;
 
 #define KBMOD_MAX_PSF 31
@@ -106,6 +107,12 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
                  const float* vel_grid, int V, int K, int min_obs,
                  const kbmod_result* out, void* workspace, size_t workspace_bytes,
                  void* stream);
+
+/* Completion status of the last kbmod_search that used this workspace.  SYNCHRONISES the stream
+ * (the one call of the library that does).  KBMOD_OK, or KBMOD_ERR_TIMEOUT if a warp of the
+ * TMA-staged kernel gave up a barrier wait after ~2 s (its results are then invalid; the kernel
+ * terminates instead of hanging the device), or KBMOD_ERR_CUDA if the stream reports a fault. */
+int kbmod_search_status(const void* workspace, void* stream);
 
 /* Bytes of device scratch kbmod_search needs for these sizes (pure function; 0 on bad sizes). */
 size_t kbmod_search_workspace(int N, int H, int W, int V, int K);

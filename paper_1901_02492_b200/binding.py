@@ -19,7 +19,7 @@ _lib: Optional[ctypes.CDLL] = None
 
 EXPORTS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_workspace", "kbmod_search_split",
            "kbmod_eval_trajectories", "kbmod_set_search_kernel", "kbmod_launch_count",
-           "kbmod_status_string", "kbmod_version", "kbmod_debug_staged_plan")
+           "kbmod_status_string", "kbmod_version", "kbmod_debug_staged_plan", "kbmod_search_status")
 
 
 class KbmodError(RuntimeError):
@@ -44,7 +44,7 @@ def lib() -> ctypes.CDLL:
         L.kbmod_version.restype = ctypes.c_char_p
         for n in ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_split",
                   "kbmod_eval_trajectories", "kbmod_set_search_kernel",
-                  "kbmod_debug_staged_plan"):
+                  "kbmod_debug_staged_plan", "kbmod_search_status"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -83,6 +83,13 @@ def launch_count() -> int:
 
 def set_search_kernel(which: int) -> None:
     _check(lib().kbmod_set_search_kernel(int(which)), "kbmod_set_search_kernel")
+
+
+def search_status(workspace: torch.Tensor) -> None:
+    """kbmod_search_status: synchronises the current stream and raises if the last search that
+    used this workspace did not complete (KBMOD_ERR_TIMEOUT / CUDA fault)."""
+    _check(lib().kbmod_search_status(_dev(workspace, torch.uint8, "workspace"), _stream()),
+           "kbmod_search_status")
 
 
 def debug_staged_plan(times, N: int, H: int, W: int, vel_grid):
@@ -154,7 +161,8 @@ def search(psiphi: torch.Tensor, times, vel_grid, K: int, min_obs: int,
     if out is None:
         out = alloc_result(H, W, K, psiphi.device)
     need = search_workspace(N, H, W, V, K)
-    if workspace is None:
+    own_workspace = workspace is None
+    if own_workspace:
         workspace = torch.empty(need, dtype=torch.uint8, device=psiphi.device)
     res = _Result(*[ctypes.c_void_p(out[k].data_ptr()) for k in
                     ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")])
@@ -168,6 +176,10 @@ def search(psiphi: torch.Tensor, times, vel_grid, K: int, min_obs: int,
                             ctypes.byref(res), _dev(workspace, torch.uint8, "workspace"),
                             ctypes.c_size_t(workspace.numel()), _stream())
     _check(rc, "kbmod_search")
+    if own_workspace:
+        # convenience path (no caller workspace to query later): wait and report a kernel that
+        # gave up; callers that pass a workspace stay asynchronous and call search_status()
+        search_status(workspace)
     return out
 
 

@@ -31,12 +31,14 @@ static bool have_device() {
 }
 
 struct WorkspaceLayout {
-    size_t vel_off, plan_off, enc_off, total;
+    size_t status_off, vel_off, plan_off, enc_off, total;
 };
 
 static WorkspaceLayout workspace_layout(int N, int H, int W, int V, int K) {
     WorkspaceLayout l;
     size_t off = 0;
+    l.status_off = off;
+    off = align_up(off + sizeof(int), 256);
     l.vel_off = off;
     off = align_up(off + (size_t)V * sizeof(float2), 256);
     l.plan_off = off;
@@ -103,12 +105,14 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
     const float2* pp = reinterpret_cast<const float2*>(psiphi);
     const int which = g_search_kernel.load();
 
+    int* status_dev = reinterpret_cast<int*>(ws + l.status_off);
+    if (cudaMemsetAsync(status_dev, 0, sizeof(int), st) != cudaSuccess) return KBMOD_ERR_CUDA;
     float2* vel_dev = reinterpret_cast<float2*>(ws + l.vel_off);
     if (cudaMemcpyAsync(vel_dev, vel_grid, (size_t)V * sizeof(float2), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
     if (which == 3)      // TMA-staged kernel: opt-in until it has been validated on hardware
         return launch_search_staged(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out, ws + l.plan_off, vel_dev,
-                                    reinterpret_cast<float2*>(ws + l.enc_off), st);
+                                    reinterpret_cast<float2*>(ws + l.enc_off), status_dev, st);
     if (which != 1) {
         const int rc = launch_search_tiled(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out,
                                            ws + l.plan_off, vel_dev,
@@ -116,6 +120,17 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
         if (rc != KBMOD_ERR_UNSUPPORTED || which == 2) return rc;
     }
     return launch_search_direct(pp, dt, N, H, W, vel_dev, V, K, min_obs, *out, st);
+}
+
+int kbmod_search_status(const void* workspace, void* stream) {
+    if (!workspace) return KBMOD_ERR_NULL;
+    if ((uintptr_t)workspace & 255) return KBMOD_ERR_ALIGN;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    int status = 0;
+    if (cudaMemcpyAsync(&status, workspace, sizeof(int), cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess ||
+        cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess)
+        return KBMOD_ERR_CUDA;
+    return status == 0 ? KBMOD_OK : KBMOD_ERR_TIMEOUT;
 }
 
 int kbmod_search_split(const float* psi, const float* phi, const double* times, int N, int H,
@@ -176,6 +191,7 @@ const char* kbmod_status_string(int status) {
         case KBMOD_ERR_CUDA: return "CUDA error or no CUDA device";
         case KBMOD_ERR_UNSUPPORTED: return "beyond the supported limits";
         case KBMOD_ERR_WORKSPACE: return "workspace too small";
+        case KBMOD_ERR_TIMEOUT: return "a kernel gave up waiting on its own pipeline";
     }
     return "unknown status";
 }

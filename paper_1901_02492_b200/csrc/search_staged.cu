@@ -332,16 +332,30 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
+    unsigned ok;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra LAB_DONE;\n"
-        "bra LAB_WAIT;\n"
-        "LAB_DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+// Warp-uniform bounded wait (all 32 lanes must call it).  A wait that lasts WAIT_LIMIT_CLOCKS
+// (about two seconds; a healthy wait is microseconds) means the pipeline is broken: the warp
+// gives up instead of hanging the GPU, and the caller reports KBMOD_ERR_TIMEOUT.
+constexpr long long WAIT_LIMIT_CLOCKS = 1ll << 32;
+__device__ __forceinline__ bool mbar_wait(unsigned bar, unsigned parity) {
+    bool ok = mbar_try_wait(bar, parity);
+    if (!ok) {
+        const long long t0 = clock64();
+        for (;;) {
+            ok = mbar_try_wait(bar, parity);
+            if (ok || clock64() - t0 > WAIT_LIMIT_CLOCKS) break;
+        }
+    }
+    return __all_sync(0xFFFFFFFFu, ok);
 }
 __device__ __forceinline__ void tma_load_3d(unsigned dst, const void* tmap, int c0, int c1, int c2, unsigned bar) {
     asm volatile(
@@ -378,6 +392,7 @@ struct StagedParams {
     const u64* enc;           // encoded stack, row pitch Wp
     const int* plan;          // nent entries of HDR_INTS ints
     const float2* vel;        // caller's velocity table (device copy)
+    int* status;              // device word: set to 1 by a warp whose barrier wait timed out
     int nent, N, H, W, Wp, K, min_obs;
     int tiles_x, tiles_y, ntiles, group_w;
     kbmod_result out;
@@ -525,7 +540,10 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
                     const bool load = (type == ENT_TMA) && !(gx + bw <= 0 || gx >= W || gy + bh <= 0 || gy >= H);
                     if (type == ENT_TMA && !load && lane == 0) hv |= FLAG_EMPTY << 8;
                     const unsigned sa = ring + slot * SLOT_BYTES;
-                    if (use > 0) mbar_wait(bar_empty + 8 * slot, (use - 1) & 1);
+                    if (use > 0 && !mbar_wait(bar_empty + 8 * slot, (use - 1) & 1)) {
+                        if (lane == 0) atomicExch(prm.status, 1);
+                        return;
+                    }
                     if (lane < HDR_INTS) asm volatile("st.shared.b32 [%0], %1;" ::"r"(sa + 4 * lane), "r"(hv) : "memory");
                     __syncwarp();
                     if (lane == 0) {
@@ -613,7 +631,10 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
             }
 
             const unsigned sa = ring + slot * SLOT_BYTES;
-            mbar_wait(bar_full + 8 * slot, phase);
+            if (!mbar_wait(bar_full + 8 * slot, phase)) {
+                if (lane == 0) atomicExch(prm.status, 1);
+                return;
+            }
             const int4 h = lds128(sa);
             const int type = h.x & 0xFF, flags = (h.x >> 8) & 0xFF;
             if (type == ENT_TMA && !(flags & FLAG_EMPTY)) {
@@ -783,7 +804,7 @@ static int launch_variant(const StagedParams& prm, const StagedMaps& maps, int g
 
 int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, int W,
                          const float* vel_host, int V, int K, int min_obs, const kbmod_result& out,
-                         void* plan_dev, const float2* vel_dev, float2* enc_dev, cudaStream_t st) {
+                         void* plan_dev, const float2* vel_dev, float2* enc_dev, int* status_dev, cudaStream_t st) {
     // limits of the int16 shift encoding, the queue's 24-bit velocity index, the TMA coordinates
     if (W > SH_LIMIT || H > SH_LIMIT || V >= (1 << 24)) return KBMOD_ERR_UNSUPPORTED;
     EncodeTiledFn enc_fn = encode_tiled_fn();
@@ -808,6 +829,7 @@ int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, 
     if (cudaMemcpyAsync(plan_dev, plan.stream.data(), plan.stream.size() * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
 
+    if (cudaMemsetAsync(status_dev, 0, sizeof(int), st) != cudaSuccess) return KBMOD_ERR_CUDA;
     const int Wp = (W + 1) & ~1;
     encode_kernel<<<148 * 8, 256, 0, st>>>(psiphi, reinterpret_cast<float4*>(enc_dev), W, Wp, (size_t)N * H);
     note_launch();
@@ -832,6 +854,7 @@ int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, 
     prm.enc = reinterpret_cast<const u64*>(enc_dev);
     prm.plan = static_cast<const int*>(plan_dev);
     prm.vel = vel_dev;
+    prm.status = status_dev;
     prm.nent = plan.nent; prm.N = N; prm.H = H; prm.W = W; prm.Wp = Wp; prm.K = K; prm.min_obs = min_obs;
     prm.tiles_x = (W + TW - 1) / TW;
     prm.tiles_y = (H + TH - 1) / TH;

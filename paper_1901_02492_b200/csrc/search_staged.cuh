@@ -13,10 +13,11 @@ size_t staged_enc_bytes(int N, int H, int W);
 // S3..S6 with host-planned integer shifts and TMA-staged shared-memory windows.  Returns
 // KBMOD_ERR_UNSUPPORTED when the shape does not fit this kernel (the caller then uses the
 // direct-gather kernel).  plan_dev / enc_dev are carved from the caller's workspace
-// (staged_plan_bytes() / staged_enc_bytes()); vel_dev is the device copy of the velocity table.
+// (staged_plan_bytes() / staged_enc_bytes()); vel_dev is the device copy of the velocity table;
+// status_dev is a device word the kernel sets to 1 if one of its barrier waits timed out.
 int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, int W,
                          const float* vel_host, int V, int K, int min_obs, const kbmod_result& out,
-                         void* plan_dev, const float2* vel_dev, float2* enc_dev, cudaStream_t st);
+                         void* plan_dev, const float2* vel_dev, float2* enc_dev, int* status_dev, cudaStream_t st);
 
 // Host-only: builds the entry stream for these inputs (test hook behind kbmod_debug_staged_plan).
 // info[0..7] = nent, HDR_INTS, nshapes, TW, TH, B, CAP (samples per slot), HDR_BYTES.
