@@ -379,7 +379,10 @@ __device__ __forceinline__ int4 lds128(unsigned a) {
     return v;
 }
 __device__ __forceinline__ void acc_add(u64& a, u64 s) {      // (Psi, -Phi) += (psi, -phi), RN each
-    asm("add.rn.f32x2 %0, %0, %1;" : "+l"(a) : "l"(s));
+    float2 fa = make_float2(__uint_as_float((unsigned)a), __uint_as_float((unsigned)(a >> 32)));
+    float2 fs = make_float2(__uint_as_float((unsigned)s), __uint_as_float((unsigned)(s >> 32)));
+    fa = __fadd2_rn(fa, fs);
+    a = (u64)__float_as_uint(fa.x) | ((u64)__float_as_uint(fa.y) << 32);
 }
 __device__ __forceinline__ bool better(float cn, int cj, float pn, int pj) {
     return cn > pn || (cn == pn && cj < pj);
