@@ -44,6 +44,7 @@ constexpr int RX = 2, RY = 2, R = RX * RY;   // pixels per thread: x = lane + 32
 constexpr int TW = 32 * RX, TH = NCW * RY;   // start-pixel tile: 64 x 30
 constexpr int THREADS = (NCW + 1) * 32;  // + 1 producer warp
 constexpr int B = 8;                     // velocities per block
+static_assert(B * R == 32, "the scoring switch of search_staged_kernel lists B*R = 32 steps");
 constexpr int CAP = 4096;                // samples per slot
 constexpr int NSLOT = 6;
 constexpr int HDR_INTS = 8 + 2 * B;
@@ -367,6 +368,9 @@ __device__ __forceinline__ u64 lds64(unsigned a) {
     u64 v;
     asm volatile("ld.shared.b64 %0, [%1+%2];" : "=l"(v) : "r"(a), "n"(OFF));
     return v;
+}
+__device__ __forceinline__ void sts32(unsigned a, int v) {
+    asm volatile("st.shared.b32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
 }
 __device__ __forceinline__ int lds32(unsigned a) {
     int v;
@@ -697,38 +701,60 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
             }
 
             if (flags & FLAG_LAST) {
-                // ---- S5 + S6 for the B x R trajectories of this block
+                // ---- S5 + S6 for the B x R trajectories of this block.  The steps are the cases of
+                // one switch so that a single copy of the batch code serves all of them: a step that
+                // fills the queue to 32 leaves the switch, the batch is processed, and the switch is
+                // re-entered at the next step.
                 fresh = true;
-#pragma unroll
-                for (int b = 0; b < B; ++b) {
-                    const int j = lds32(sa + 32 + 4 * B + 4 * b);
-                    if (j < 0) continue;
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        const float Psi = __uint_as_float((unsigned)acc[b][r]);
-                        const float Phi = 0.0f - __uint_as_float((unsigned)(acc[b][r] >> 32));
-                        unsigned n;
-                        if constexpr (CM == 2) n = __popc(cnt[b][r / RX] & ((r % RX) ? 0x55555555u : 0xAAAAAAAAu));
-                        else if constexpr (CM == 1) n = __popc(cnt[b][r]);
-                        else n = cnt[b][r];
-                        const bool pass = (n >= minobs) && (Phi > 0.0f) && ((inimg >> r) & 1u) &&
-                                          !(Psi * rsqrtf(Phi) < lo[r]);
-                        const unsigned m = __ballot_sync(0xFFFFFFFFu, pass);
-                        if (m) {
-                            if (pass) {
-                                const unsigned qi = (qtail + __popc(m & ((1u << lane) - 1u))) & (QCAP - 1);
-                                asm volatile("st.shared.b32 [%0], %1;" ::"r"(qb + 4 * qi), "r"(__float_as_int(Psi)) : "memory");
-                                asm volatile("st.shared.b32 [%0], %1;" ::"r"(qb + 4 * QCAP + 4 * qi), "r"(__float_as_int(Phi)) : "memory");
-                                asm volatile("st.shared.b32 [%0], %1;" ::"r"(qb + 8 * QCAP + 4 * qi), "r"((j << 7) | (r << 5) | lane) : "memory");
-                            }
-                            qtail += __popc(m);
-                            __syncwarp();
-                            if (qtail - qhead >= 32) {
-                                process_batch<KP>(prm, qb, qhead, 32, lane, tile_x, y_first);
-                                qhead += 32;
-                            }
-                        }
+                int step = 0;
+                for (;;) {
+                    bool flush = false;
+                    switch (step) {
+#define KBMOD_SCORE_STEP(S)                                                                              \
+    case S: {                                                                                            \
+        constexpr int b_ = (S) / R, r_ = (S) % R;                                                        \
+        const int j = lds32(sa + 32 + 4 * B + 4 * b_);                                                   \
+        if (j >= 0) {                                                                                    \
+            const float Psi = __uint_as_float((unsigned)acc[b_][r_]);                                    \
+            const float Phi = 0.0f - __uint_as_float((unsigned)(acc[b_][r_] >> 32));                     \
+            unsigned n;                                                                                  \
+            if constexpr (CM == 2) n = __popc(cnt[b_][r_ / RX] & ((r_ % RX) ? 0x55555555u : 0xAAAAAAAAu)); \
+            else if constexpr (CM == 1) n = __popc(cnt[b_][r_ % NC]);                                    \
+            else n = cnt[b_][r_ % NC];                                                                   \
+            const bool pass = (n >= minobs) && (Phi > 0.0f) && ((inimg >> r_) & 1u) &&                   \
+                              !(Psi * rsqrtf(Phi) < lo[r_]);                                             \
+            const unsigned m = __ballot_sync(0xFFFFFFFFu, pass);                                         \
+            if (m) {                                                                                     \
+                if (pass) {                                                                              \
+                    const unsigned qi = (qtail + __popc(m & ((1u << lane) - 1u))) & (QCAP - 1);          \
+                    sts32(qb + 4 * qi, __float_as_int(Psi));                                             \
+                    sts32(qb + 4 * QCAP + 4 * qi, __float_as_int(Phi));                                  \
+                    sts32(qb + 8 * QCAP + 4 * qi, (j << 7) | (r_ << 5) | lane);                          \
+                }                                                                                        \
+                qtail += __popc(m);                                                                      \
+                if (qtail - qhead >= 32) {                                                               \
+                    step = (S) + 1;                                                                      \
+                    flush = true;                                                                        \
+                    break;                                                                               \
+                }                                                                                        \
+            }                                                                                            \
+        }                                                                                                \
+    }
+                        KBMOD_SCORE_STEP(0) KBMOD_SCORE_STEP(1) KBMOD_SCORE_STEP(2) KBMOD_SCORE_STEP(3)
+                        KBMOD_SCORE_STEP(4) KBMOD_SCORE_STEP(5) KBMOD_SCORE_STEP(6) KBMOD_SCORE_STEP(7)
+                        KBMOD_SCORE_STEP(8) KBMOD_SCORE_STEP(9) KBMOD_SCORE_STEP(10) KBMOD_SCORE_STEP(11)
+                        KBMOD_SCORE_STEP(12) KBMOD_SCORE_STEP(13) KBMOD_SCORE_STEP(14) KBMOD_SCORE_STEP(15)
+                        KBMOD_SCORE_STEP(16) KBMOD_SCORE_STEP(17) KBMOD_SCORE_STEP(18) KBMOD_SCORE_STEP(19)
+                        KBMOD_SCORE_STEP(20) KBMOD_SCORE_STEP(21) KBMOD_SCORE_STEP(22) KBMOD_SCORE_STEP(23)
+                        KBMOD_SCORE_STEP(24) KBMOD_SCORE_STEP(25) KBMOD_SCORE_STEP(26) KBMOD_SCORE_STEP(27)
+                        KBMOD_SCORE_STEP(28) KBMOD_SCORE_STEP(29) KBMOD_SCORE_STEP(30) KBMOD_SCORE_STEP(31)
+#undef KBMOD_SCORE_STEP
+                        default: break;
                     }
+                    if (!flush) break;
+                    __syncwarp();
+                    process_batch<KP>(prm, qb, qhead, 32, lane, tile_x, y_first);
+                    qhead += 32;
                 }
             }
             __syncwarp();
