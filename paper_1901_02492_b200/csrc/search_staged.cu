@@ -11,13 +11,13 @@
 //     packed add.rn.f32x2 accumulates both sums (adding zero is exact, so the result equals the
 //     in-order fp32 sum over the valid observations), the sign bit of the second word is the
 //     validity flag, and TMA's zero fill outside the image IS the "no observation" sample.
-//   * A persistent CTA (one per SM) owns a 64x32 tile of start pixels at a time and walks the
+//   * A persistent CTA (one per SM) owns a 64x30 tile of start pixels at a time and walks the
 //     velocity grid in blocks of B = 8 velocities that are neighbours in the (vx,vy) plane
 //     (Hilbert order).  Every thread keeps Psi/Phi/validity history of 8 velocities x 4 pixels in
 //     registers.  For each image the host has grouped the block's 8 shifted windows into
 //     bounding boxes that fit a shared-memory slot; a producer warp streams these boxes with
 //     cp.async.bulk.tensor (TMA, 3-D tensor map over [N][H][W], zero fill) into a ring of slots
-//     guarded by full/empty mbarriers, and 16 consumer warps read them with conflict-free
+//     guarded by full/empty mbarriers, and 15 consumer warps read them with conflict-free
 //     LDS.64: 3 instructions per sample (LDS.64, FADD2, SHF).
 //   * S5/S6: an approximate Psi*rsqrt(Phi) test against the pixel's current K-th best keeps
 //     almost every trajectory off the exact path.  Survivors are compacted into a per-warp
@@ -26,6 +26,7 @@
 //     Psi/Phi/n_obs/alpha of the K winners are re-evaluated literally at the end of the tile.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <vector>
@@ -45,14 +46,18 @@ constexpr int TW = 32 * RX, TH = NCW * RY;   // start-pixel tile: 64 x 30
 constexpr int THREADS = (NCW + 1) * 32;  // + 1 producer warp
 constexpr int B = 8;                     // velocities per block
 static_assert(B * R == 32, "the scoring switch of search_staged_kernel lists B*R = 32 steps");
-constexpr int CAP = 4096;                // samples per slot
-constexpr int NSLOT = 6;
+// ring geometry variants (samples per slot, slots); selected per call by the environment variable
+// KBMOD_STAGED_GEOM (tuning knob; default 0).  Smaller slots = more boxes in flight but fewer
+// windows merged per box.
+constexpr int NGEOM = 4;
+__host__ __device__ constexpr int cap_of(int g) { return g == 0 ? 4096 : g == 1 ? 3072 : g == 2 ? 6144 : 2560; }
+__host__ __device__ constexpr int nslot_of(int g) { return g == 0 ? 6 : g == 1 ? 8 : g == 2 ? 4 : 10; }
 constexpr int HDR_INTS = 8 + 2 * B;
 constexpr int HDR_BYTES = 128;
 static_assert(HDR_INTS * 4 <= HDR_BYTES, "header");
-constexpr int SLOT_BYTES = HDR_BYTES + CAP * 8;
+__host__ __device__ constexpr int slot_bytes_of(int g) { return HDR_BYTES + cap_of(g) * 8; }
 constexpr int QCAP = 64;                 // per-warp candidate queue entries
-constexpr int MAXMAPS = 160;
+constexpr int MAXMAPS = 240;             // 240 x 128 B of tensor maps + the other parameters stay below the 32764-byte limit
 constexpr int MAXBW = 128;               // box width limit (256 fp32 elements per TMA box row)
 constexpr int SH_LIMIT = 30000;
 
@@ -65,7 +70,17 @@ constexpr int SH_LIMIT = 30000;
 enum { ENT_NOP = 0, ENT_TMA = 1, ENT_UNSAFE = 2 };
 enum { FLAG_LAST = 1, FLAG_EMPTY = 2 };
 
-constexpr size_t SMEM_BYTES = (size_t)NSLOT * SLOT_BYTES + (size_t)NCW * QCAP * 12 + 2 * NSLOT * 8;
+constexpr size_t smem_bytes_of(int g) {
+    return (size_t)nslot_of(g) * slot_bytes_of(g) + (size_t)NCW * QCAP * 12 + 2 * nslot_of(g) * 8;
+}
+static_assert(smem_bytes_of(0) <= 227 * 1024 && smem_bytes_of(1) <= 227 * 1024 && smem_bytes_of(2) <= 227 * 1024 &&
+              smem_bytes_of(3) <= 227 * 1024, "ring does not fit shared memory");
+
+int staged_geom() {                       // KBMOD_STAGED_GEOM in [0, NGEOM), else 0
+    const char* e = std::getenv("KBMOD_STAGED_GEOM");
+    if (!e || e[0] < '0' || e[0] >= '0' + NGEOM || e[1] != 0) return 0;
+    return e[0] - '0';
+}
 
 unsigned hilbert_d(unsigned x, unsigned y) {   // Hilbert index of a 16-bit quantised (x, y)
     unsigned d = 0;
@@ -134,7 +149,7 @@ inline void box_of(const Group& g, const BoxQ& q, int& ox, int& bw, int& bh) {
     bh = g.syhi - g.sylo + TH;
     bh = (bh + q.qh - 1) / q.qh * q.qh;
 }
-inline bool box_fits(int bw, int bh) { return bw <= MAXBW && bh <= 256 && bw * bh <= CAP; }
+inline bool box_fits(int bw, int bh, int cap) { return bw <= MAXBW && bh <= 256 && bw * bh <= cap; }
 
 }  // namespace
 
@@ -143,12 +158,12 @@ struct StagedPlan {
     std::vector<std::pair<int, int>> shapes; // distinct (bw, bh); index = tensor-map id
     int nent = 0;
     // key
-    int N = 0, H = 0, W = 0, V = 0;
+    int N = 0, H = 0, W = 0, V = 0, cap = 0;
     std::vector<float> dt, vel;
 };
 
 // Builds the entry stream.  Returns false when the box shapes cannot be brought under MAXMAPS.
-static bool build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, StagedPlan& plan) {
+static bool build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, int cap, StagedPlan& plan) {
     // processing order: Hilbert curve over the velocity plane (ties: index)
     float lox = vel[0], hix = vel[0], loy = vel[1], hiy = vel[1];
     for (int j = 1; j < V; ++j) {
@@ -221,7 +236,7 @@ static bool build_plan(const DtTable& dt, int N, int H, int W, const float* vel,
                                     std::max(groups[a].syhi, groups[c].syhi)};
                             int ox, bw, bh, wa, ha, wc, hc;
                             box_of(m, q, ox, bw, bh);
-                            if (!box_fits(bw, bh)) continue;
+                            if (!box_fits(bw, bh, cap)) continue;
                             box_of(groups[a], q, ox, wa, ha);
                             box_of(groups[c], q, ox, wc, hc);
                             const int save = wa * ha + wc * hc - bw * bh;
@@ -237,7 +252,7 @@ static bool build_plan(const DtTable& dt, int N, int H, int W, const float* vel,
                 for (const Group& g : groups) {
                     int ox, bw, bh;
                     box_of(g, q, ox, bw, bh);
-                    if (!box_fits(bw, bh)) { too_many = true; break; }   // quantised singleton too big
+                    if (!box_fits(bw, bh, cap)) { too_many = true; break; }   // quantised singleton too big
                     int id = -1;
                     for (size_t m = 0; m < plan.shapes.size(); ++m)
                         if (plan.shapes[m].first == bw && plan.shapes[m].second == bh) { id = (int)m; break; }
@@ -282,9 +297,10 @@ int staged_plan_debug(const DtTable& dt, int N, int H, int W, const float* vel_h
                       int32_t* stream, size_t stream_ints, int32_t* shapes, int max_shapes, int32_t* info) {
     if (W > SH_LIMIT || H > SH_LIMIT || V >= (1 << 24)) return KBMOD_ERR_UNSUPPORTED;
     StagedPlan plan;
-    if (!build_plan(dt, N, H, W, vel_host, V, plan)) return KBMOD_ERR_UNSUPPORTED;
+    const int cap = cap_of(staged_geom());
+    if (!build_plan(dt, N, H, W, vel_host, V, cap, plan)) return KBMOD_ERR_UNSUPPORTED;
     info[0] = plan.nent; info[1] = HDR_INTS; info[2] = (int)plan.shapes.size(); info[3] = TW;
-    info[4] = TH; info[5] = B; info[6] = CAP; info[7] = HDR_BYTES;
+    info[4] = TH; info[5] = B; info[6] = cap; info[7] = HDR_BYTES;
     if (plan.stream.size() * sizeof(int) > staged_plan_bytes(N, V)) return KBMOD_ERR_UNSUPPORTED;
     if (plan.stream.size() > stream_ints || (int)plan.shapes.size() > max_shapes) return KBMOD_ERR_WORKSPACE;
     std::memcpy(stream, plan.stream.data(), plan.stream.size() * sizeof(int));
@@ -496,11 +512,14 @@ __device__ __forceinline__ void coadd_literal(const StagedParams& prm, int x0, i
     }
 }
 
+static_assert(sizeof(StagedParams) + sizeof(StagedMaps) <= 32764, "kernel parameters exceed the 32764-byte limit");
+
 // CM: how the validity of the samples is counted.  2: history bits, the two rx pixels of a row
 // share a register (N <= 16); 1: history bits, one register per pixel (N <= 32); 0: additive.
-template <int CM, int KP>
+template <int CM, int KP, int G>
 __global__ void __launch_bounds__(THREADS, 1)
 search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_constant__ StagedMaps maps) {
+    constexpr int NSLOT = nslot_of(G), SLOT_BYTES = slot_bytes_of(G);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const unsigned ring = smem_u32(smem_raw);
     const unsigned qall = ring + NSLOT * SLOT_BYTES;
@@ -817,18 +836,27 @@ static EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
-template <int CM, int KP>
+template <int CM, int KP, int G>
 static int launch_variant(const StagedParams& prm, const StagedMaps& maps, int grid, cudaStream_t st) {
-    auto kern = search_staged_kernel<CM, KP>;
+    auto kern = search_staged_kernel<CM, KP, G>;
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes_of(G)) != cudaSuccess)
             return KBMOD_ERR_CUDA;
         attr_set = true;
     }
-    kern<<<grid, THREADS, SMEM_BYTES, st>>>(prm, maps);
+    kern<<<grid, THREADS, smem_bytes_of(G), st>>>(prm, maps);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
+}
+template <int CM, int KP>
+static int launch_geom(int g, const StagedParams& prm, const StagedMaps& maps, int grid, cudaStream_t st) {
+    switch (g) {
+        case 1: return launch_variant<CM, KP, 1>(prm, maps, grid, st);
+        case 2: return launch_variant<CM, KP, 2>(prm, maps, grid, st);
+        case 3: return launch_variant<CM, KP, 3>(prm, maps, grid, st);
+        default: return launch_variant<CM, KP, 0>(prm, maps, grid, st);
+    }
 }
 
 int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, int W,
@@ -843,13 +871,14 @@ int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, 
     static std::mutex mu;
     static StagedPlan cached;
     std::lock_guard<std::mutex> lock(mu);
-    const bool hit = cached.nent > 0 && cached.N == N && cached.H == H && cached.W == W && cached.V == V &&
+    const int geom = staged_geom(), cap = cap_of(geom);
+    const bool hit = cached.nent > 0 && cached.cap == cap && cached.N == N && cached.H == H && cached.W == W && cached.V == V &&
                      std::memcmp(cached.dt.data(), dt.dt, sizeof(float) * N) == 0 &&
                      std::memcmp(cached.vel.data(), vel_host, sizeof(float) * 2 * V) == 0;
     if (!hit) {
         cached.nent = 0;
-        if (!build_plan(dt, N, H, W, vel_host, V, cached)) return KBMOD_ERR_UNSUPPORTED;
-        cached.N = N; cached.H = H; cached.W = W; cached.V = V;
+        if (!build_plan(dt, N, H, W, vel_host, V, cap, cached)) return KBMOD_ERR_UNSUPPORTED;
+        cached.cap = cap; cached.N = N; cached.H = H; cached.W = W; cached.V = V;
         cached.dt.assign(dt.dt, dt.dt + N);
         cached.vel.assign(vel_host, vel_host + 2 * (size_t)V);
     }
@@ -899,12 +928,12 @@ int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, 
     const int grid = (int)std::min<long long>(tiles, sms);
     const int cm = N <= 16 ? 2 : (N <= 32 ? 1 : 0);
     if (K <= 8) {
-        if (cm == 2) return launch_variant<2, 8>(prm, maps, grid, st);
-        if (cm == 1) return launch_variant<1, 8>(prm, maps, grid, st);
-        return launch_variant<0, 8>(prm, maps, grid, st);
+        if (cm == 2) return launch_geom<2, 8>(geom, prm, maps, grid, st);
+        if (cm == 1) return launch_geom<1, 8>(geom, prm, maps, grid, st);
+        return launch_geom<0, 8>(geom, prm, maps, grid, st);
     }
-    if (cm == 2) return launch_variant<2, 0>(prm, maps, grid, st);
-    if (cm == 1) return launch_variant<1, 0>(prm, maps, grid, st);
-    return launch_variant<0, 0>(prm, maps, grid, st);
+    if (cm == 2) return launch_geom<2, 0>(geom, prm, maps, grid, st);
+    if (cm == 1) return launch_geom<1, 0>(geom, prm, maps, grid, st);
+    return launch_geom<0, 0>(geom, prm, maps, grid, st);
 }
 }  // namespace kbmod

@@ -142,6 +142,18 @@ def test_plan_reproduces_oracle_on_crops(orc, k, over):
     check_against_oracle(orc, pp, st.times, st.vel_grid)
 
 
+@pytest.mark.parametrize("geom", ["1", "2", "3"])
+def test_plan_ring_geometry_variants(orc, geom, monkeypatch):
+    """KBMOD_STAGED_GEOM selects other slot sizes: the plan must stay exact and respect the cap."""
+    monkeypatch.setenv("KBMOD_STAGED_GEOM", geom)
+    cfg = synth.config(3, N=15, H=70, W=133, n_sources=4)
+    st = synth.make_stack(cfg)
+    pp = orc.make_psi_phi(st.sci, st.var, st.mask, st.psf)
+    _, _, info = binding.debug_staged_plan(st.times, cfg.N, cfg.H, cfg.W, st.vel_grid)
+    assert info["CAP"] == {"1": 3072, "2": 6144, "3": 2560}[geom]
+    check_against_oracle(orc, pp, st.times, st.vel_grid)
+
+
 def test_plan_interior_trajectories(orc):
     pp = synth.random_psiphi(9, 95, 200, seed=21, invalid_frac=0.03)
     times = np.array([0, .05, .1, .15, 1, 1.05, 1.1, 2.0, 2.05])
