@@ -34,6 +34,7 @@
 #include <cuda.h>
 
 #include "search_staged.cuh"
+#include "topk_list.h"
 
 namespace kbmod {
 
@@ -404,10 +405,6 @@ __device__ __forceinline__ void acc_add(u64& a, u64 s) {      // (Psi, -Phi) += 
     fa = __fadd2_rn(fa, fs);
     a = (u64)__float_as_uint(fa.x) | ((u64)__float_as_uint(fa.y) << 32);
 }
-__device__ __forceinline__ bool better(float cn, int cj, float pn, int pj) {
-    return cn > pn || (cn == pn && cj < pj);
-}
-
 struct StagedMaps { CUtensorMap m[MAXMAPS]; };
 
 struct StagedParams {
@@ -434,44 +431,12 @@ __device__ __forceinline__ void tile_of(const StagedParams& prm, int t, int& til
     tile_y = ty * TH;
 }
 
-// ---- S6: sorted insert of (nu, j) into one pixel's list (nu descending, ties: smaller j first).
-// The list is the pixel's K slots of the nu / vel_idx output planes; only the owning warp touches it.
-template <int KP>
-__device__ __forceinline__ void list_insert(float* Ln, int* Lj, int K, float cn, int cj) {
-    if constexpr (KP > 0) {            // K <= KP: whole list in registers, one round trip
-        float ln[KP];
-        int lj[KP];
-#pragma unroll
-        for (int e = 0; e < KP; ++e) {
-            ln[e] = (e < K) ? __ldcg(Ln + e) : INFINITY;
-            lj[e] = (e < K) ? __ldcg(Lj + e) : -1;
-        }
-        bool gt[KP];
-#pragma unroll
-        for (int e = 0; e < KP; ++e) gt[e] = better(cn, cj, ln[e], lj[e]);
-#pragma unroll
-        for (int e = KP - 1; e >= 0; --e) {
-            if (e < K && gt[e]) {
-                const bool shift = (e > 0) && gt[e > 0 ? e - 1 : 0];
-                __stcg(Ln + e, shift ? ln[e > 0 ? e - 1 : 0] : cn);
-                __stcg(Lj + e, shift ? lj[e > 0 ? e - 1 : 0] : cj);
-            }
-        }
-    } else {
-        if (!better(cn, cj, __ldcg(Ln + K - 1), __ldcg(Lj + K - 1))) return;
-        int e = K - 1;
-        while (e > 0) {
-            const float pn = __ldcg(Ln + e - 1);
-            const int pj = __ldcg(Lj + e - 1);
-            if (!better(cn, cj, pn, pj)) break;
-            __stcg(Ln + e, pn);
-            __stcg(Lj + e, pj);
-            --e;
-        }
-        __stcg(Ln + e, cn);
-        __stcg(Lj + e, cj);
-    }
-}
+// memory policy of the per-pixel lists: they live in the nu / vel_idx output planes and are read
+// and written through L2 (only the owning warp touches a pixel's list)
+struct ListMemL2 {
+    template <class T> static __device__ __forceinline__ T ld(const T* p) { return __ldcg(p); }
+    template <class T> static __device__ __forceinline__ void st(T* p, T v) { __stcg(p, v); }
+};
 
 // One dense pass over up to 32 queued candidates of this warp: lane l takes entry qhead + l.
 template <int KP>
@@ -491,7 +456,7 @@ __device__ __forceinline__ void process_batch(const StagedParams& prm, unsigned 
         // two candidates of the same pixel in one batch: lowest lane first, the rest next round
         const unsigned same = __match_any_sync(0xFFFFFFFFu, valid ? pix : 128 + lane);
         if (valid && lane == __ffs(same) - 1) {
-            list_insert<KP>(prm.out.nu + p, prm.out.vel_idx + p, prm.K, nu, j);
+            list_insert<KP, ListMemL2>(prm.out.nu + p, prm.out.vel_idx + p, prm.K, nu, j);
             valid = false;
         }
         __syncwarp();
@@ -615,7 +580,7 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
                 const size_t p = (pix0 + 32 * (r % RX) + (size_t)(r / RX) * W) * K;
                 for (int kk = 0; kk < K; ++kk) {
                     __stcg(prm.out.nu + p + kk, -INFINITY);
-                    __stcg(prm.out.vel_idx + p + kk, 0x7FFFFFFF);
+                    __stcg(prm.out.vel_idx + p + kk, LIST_EMPTY_IDX);
                 }
             }
         __syncwarp();
@@ -795,7 +760,7 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
             const size_t p = ((size_t)y0 * W + x0) * K;
             for (int kk = 0; kk < K; ++kk) {
                 const int j = __ldcg(prm.out.vel_idx + p + kk);
-                if (j != 0x7FFFFFFF) {
+                if (j != LIST_EMPTY_IDX) {
                     float Psi, Phi;
                     int n;
                     coadd_literal(prm, x0, y0, __ldg(prm.vel + j), Psi, Phi, n);
