@@ -33,6 +33,7 @@
 
 #include <cuda.h>
 
+#include "ring_alloc.h"
 #include "search_staged.cuh"
 #include "topk_list.h"
 
@@ -50,9 +51,17 @@ static_assert(B * R == 32, "the scoring switch of search_staged_kernel lists B*R
 // ring geometry variants (samples per slot, slots); selected per call by the environment variable
 // KBMOD_STAGED_GEOM (tuning knob; default 0).  Smaller slots = more boxes in flight but fewer
 // windows merged per box.
-constexpr int NGEOM = 4;
-__host__ __device__ constexpr int cap_of(int g) { return g == 0 ? 4096 : g == 1 ? 3072 : g == 2 ? 6144 : 2560; }
-__host__ __device__ constexpr int nslot_of(int g) { return g == 0 ? 6 : g == 1 ? 8 : g == 2 ? 4 : 10; }
+// Geometries 0-3: ring of equal slots (header + box).  Geometries 4-6: byte-granular data ring
+// (ring_alloc.h) with a separate ring of VR_NH headers, so that the boxes in flight fill the
+// whole shared memory whatever their sizes; cap = largest box.
+constexpr int NGEOM = 7;
+__host__ __device__ constexpr int cap_of(int g) {
+    return g == 0 ? 4096 : g == 1 ? 3072 : g == 2 ? 6144 : g == 3 ? 2560 : g == 4 ? 4096 : g == 5 ? 6144 : 8192;
+}
+__host__ __device__ constexpr bool is_var(int g) { return g >= 4; }
+constexpr int VR_NH = 16;                // header slots (= entries in flight at most) of the variable ring
+constexpr int VR_RING_BYTES = 212992;    // data bytes of the variable ring (208 KB)
+__host__ __device__ constexpr int nslot_of(int g) { return g == 0 ? 6 : g == 1 ? 8 : g == 2 ? 4 : g == 3 ? 10 : VR_NH; }
 constexpr int HDR_INTS = 8 + 2 * B;
 constexpr int HDR_BYTES = 128;
 static_assert(HDR_INTS * 4 <= HDR_BYTES, "header");
@@ -65,17 +74,25 @@ constexpr int SH_LIMIT = 30000;
 // entry header (ints)
 //  [0] type | flags << 8 | image << 16     [1] member mask      [2] row pitch of the box, bytes
 //  [3] ox | oy << 16 (int16, box origin - tile origin)          [4] bw | bh << 16
-//  [5] tensor-map id (ENT_TMA) / member b (ENT_UNSAFE)          [6],[7] vx, vy bits (ENT_UNSAFE)
-//  [8 .. 8+B)    byte offset (from the slot base) of member b's window origin
+//  [5] tensor-map id (ENT_TMA) / member b (ENT_UNSAFE)          [6],[7] vx, vy bits (ENT_UNSAFE);
+//      on ENT_TMA entries the producer stores the box's byte offset in the data ring in [6]
+//  [8 .. 8+B)    byte offset (from the box start) of member b's window origin
 //  [8+B .. 8+2B) original velocity index of member b, -1 = padding (read on FLAG_LAST entries)
 enum { ENT_NOP = 0, ENT_TMA = 1, ENT_UNSAFE = 2 };
 enum { FLAG_LAST = 1, FLAG_EMPTY = 2 };
 
+// shared memory: [ring][queues][full barriers][empty barriers][adv table]; ring = slots (fixed) or
+// data bytes followed by the headers (variable)
+__host__ __device__ constexpr size_t ring_bytes_of(int g) {
+    return is_var(g) ? (size_t)VR_RING_BYTES + (size_t)VR_NH * HDR_BYTES : (size_t)nslot_of(g) * slot_bytes_of(g);
+}
 constexpr size_t smem_bytes_of(int g) {
-    return (size_t)nslot_of(g) * slot_bytes_of(g) + (size_t)NCW * QCAP * 12 + 2 * nslot_of(g) * 8;
+    return ring_bytes_of(g) + (size_t)NCW * QCAP * 12 + 2 * nslot_of(g) * 8 + VR_NH * 4;
 }
 static_assert(smem_bytes_of(0) <= 227 * 1024 && smem_bytes_of(1) <= 227 * 1024 && smem_bytes_of(2) <= 227 * 1024 &&
-              smem_bytes_of(3) <= 227 * 1024, "ring does not fit shared memory");
+              smem_bytes_of(3) <= 227 * 1024 && smem_bytes_of(4) <= 227 * 1024 && smem_bytes_of(6) <= 227 * 1024,
+              "ring does not fit shared memory");
+static_assert(cap_of(6) * 8 <= VR_RING_BYTES / 2, "a box must fit the variable ring comfortably");
 
 int staged_geom() {                       // KBMOD_STAGED_GEOM in [0, NGEOM), else 0
     const char* e = std::getenv("KBMOD_STAGED_GEOM");
@@ -271,7 +288,7 @@ static bool build_plan(const DtTable& dt, int N, int H, int W, const float* vel,
                     for (int b = 0; b < B; ++b)
                         if (g.mask & (1u << b)) {
                             const size_t k = (size_t)jb[b] * N + i;
-                            e[8 + b] = HDR_BYTES + ((shy[k] - g.sylo) * bw + (shx[k] - ox)) * 8;
+                            e[8 + b] = ((shy[k] - g.sylo) * bw + (shx[k] - ox)) * 8;
                         }
                 }
                 if (too_many) break;
@@ -484,12 +501,17 @@ static_assert(sizeof(StagedParams) + sizeof(StagedMaps) <= 32764, "kernel parame
 template <int CM, int KP, int G>
 __global__ void __launch_bounds__(THREADS, 1)
 search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_constant__ StagedMaps maps) {
+    constexpr bool VR = is_var(G);                    // byte-granular data ring + header ring
     constexpr int NSLOT = nslot_of(G), SLOT_BYTES = slot_bytes_of(G);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const unsigned ring = smem_u32(smem_raw);
-    const unsigned qall = ring + NSLOT * SLOT_BYTES;
+    const unsigned hdrs = ring + VR_RING_BYTES;       // VR only: NSLOT headers of HDR_BYTES
+    const unsigned qall = ring + (unsigned)ring_bytes_of(G);
     const unsigned bar_full = qall + NCW * QCAP * 12;
     const unsigned bar_empty = bar_full + NSLOT * 8;
+    // header and box of ring slot s (fixed geometry: the box follows its header; variable: the
+    // box sits in the data ring at the offset the producer stored in header int 6)
+    auto hdr_of = [&](unsigned s) -> unsigned { return VR ? hdrs + s * HDR_BYTES : ring + s * SLOT_BYTES; };
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = prm.N, H = prm.H, W = prm.W, K = prm.K;
 
@@ -515,6 +537,10 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
         int e = 0, k = 0, tile_x = 0, tile_y = 0;
         if (my_tiles > 0) tile_of(prm, blockIdx.x, tile_x, tile_y);
         unsigned slot = 0, use = 0;
+        // VR: allocator state (identical in all lanes; adv[] in shared memory) and the ring slot /
+        // phase of the oldest entry not yet released
+        RingAlloc<VR_RING_BYTES, VR_NH> ra(reinterpret_cast<unsigned*>(smem_raw + (bar_empty - ring) + NSLOT * 8));
+        unsigned oslot = 0, ophase = 0;
         for (long long g0 = 0; g0 < total; g0 += PF) {
 #pragma unroll
             for (int p = 0; p < PF; ++p) {
@@ -530,17 +556,36 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
                     const int gx = tile_x + (short)(h3 & 0xFFFF), gy = tile_y + (h3 >> 16);
                     const bool load = (type == ENT_TMA) && !(gx + bw <= 0 || gx >= W || gy + bh <= 0 || gy >= H);
                     if (type == ENT_TMA && !load && lane == 0) hv |= FLAG_EMPTY << 8;
-                    const unsigned sa = ring + slot * SLOT_BYTES;
-                    if (use > 0 && !mbar_wait(bar_empty + 8 * slot, (use - 1) & 1)) {
-                        if (lane == 0) atomicExch(prm.status, 1);
-                        return;
+                    const unsigned sa = hdr_of(slot);
+                    unsigned box_at;
+                    if constexpr (VR) {
+                        // place the box in the data ring; release finished entries (in order) until it fits
+                        const unsigned need = load ? (((unsigned)(bw * bh * 8) + 127u) & ~127u) : 0u;
+                        while (!ra.fits(need)) {
+                            if (!mbar_wait(bar_empty + 8 * oslot, ophase)) {
+                                if (lane == 0) atomicExch(prm.status, 1);
+                                return;
+                            }
+                            ra.release_oldest();
+                            if (++oslot == NSLOT) { oslot = 0; ophase ^= 1; }
+                        }
+                        const unsigned off = ra.place(need);
+                        box_at = ring + off;
+                        if (type == ENT_TMA && lane == 6) hv = (int)off;
+                    } else {
+                        if (use > 0 && !mbar_wait(bar_empty + 8 * slot, (use - 1) & 1)) {
+                            if (lane == 0) atomicExch(prm.status, 1);
+                            return;
+                        }
+                        box_at = sa + HDR_BYTES;
+                        if (type == ENT_TMA && lane == 6) hv = HDR_BYTES + (int)(slot * SLOT_BYTES);
                     }
                     if (lane < HDR_INTS) asm volatile("st.shared.b32 [%0], %1;" ::"r"(sa + 4 * lane), "r"(hv) : "memory");
                     __syncwarp();
                     if (lane == 0) {
                         if (load) {
                             mbar_arrive_expect_tx(bar_full + 8 * slot, (unsigned)(bw * bh * 8));
-                            tma_load_3d(sa + HDR_BYTES, &maps.m[h5], 2 * gx, gy, img, bar_full + 8 * slot);
+                            tma_load_3d(box_at, &maps.m[h5], 2 * gx, gy, img, bar_full + 8 * slot);
                         } else {
                             mbar_arrive(bar_full + 8 * slot);
                         }
@@ -621,7 +666,7 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
                 }
             }
 
-            const unsigned sa = ring + slot * SLOT_BYTES;
+            const unsigned sa = hdr_of(slot);
             if (!mbar_wait(bar_full + 8 * slot, phase)) {
                 if (lane == 0) atomicExch(prm.status, 1);
                 return;
@@ -630,7 +675,8 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
             const int type = h.x & 0xFF, flags = (h.x >> 8) & 0xFF;
             if (type == ENT_TMA && !(flags & FLAG_EMPTY)) {
                 const unsigned pitch = (unsigned)h.z;
-                const unsigned thr = sa + lane * 8 + (unsigned)(warp * RY) * pitch;
+                // header int 6 = byte offset of the box from the start of the ring (both geometries)
+                const unsigned thr = ring + (unsigned)lds32(sa + 24) + lane * 8 + (unsigned)(warp * RY) * pitch;
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
                     if (h.y & (1 << b)) {
@@ -820,6 +866,9 @@ static int launch_geom(int g, const StagedParams& prm, const StagedMaps& maps, i
         case 1: return launch_variant<CM, KP, 1>(prm, maps, grid, st);
         case 2: return launch_variant<CM, KP, 2>(prm, maps, grid, st);
         case 3: return launch_variant<CM, KP, 3>(prm, maps, grid, st);
+        case 4: return launch_variant<CM, KP, 4>(prm, maps, grid, st);
+        case 5: return launch_variant<CM, KP, 5>(prm, maps, grid, st);
+        case 6: return launch_variant<CM, KP, 6>(prm, maps, grid, st);
         default: return launch_variant<CM, KP, 0>(prm, maps, grid, st);
     }
 }

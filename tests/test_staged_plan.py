@@ -55,7 +55,7 @@ def run_plan(pp, times, vel, tiles=None):
     shape [TH, TW, V] (only pixels inside the image are meaningful)."""
     N, H, W, _ = pp.shape
     stream, shapes, info = binding.debug_staged_plan(times, N, H, W, vel)
-    TW, TH, B, HB = info["TW"], info["TH"], info["B"], info["HDR_BYTES"]
+    TW, TH, B = info["TW"], info["TH"], info["B"]
     enc = encode(pp)
     dt = (np.asarray(times, np.float64) - float(times[0])).astype(np.float32)
     V = vel.shape[0]
@@ -89,7 +89,7 @@ def run_plan(pp, times, vel, tiles=None):
                 box = fetch_box(enc, img, tile_x + ox, tile_y + oy, bw, bh).reshape(-1, 2)
                 for b in range(B):
                     if e[1] >> b & 1:
-                        off = e[8 + b] - HB
+                        off = e[8 + b]                         # bytes from the box start
                         assert off >= 0 and off % 8 == 0
                         idx = off // 8 + py * bw + px          # thread address: + row*pitch + x*8
                         assert idx.max() < bw * bh, "window leaves the box"
@@ -142,7 +142,7 @@ def test_plan_reproduces_oracle_on_crops(orc, k, over):
     check_against_oracle(orc, pp, st.times, st.vel_grid)
 
 
-@pytest.mark.parametrize("geom", ["1", "2", "3"])
+@pytest.mark.parametrize("geom", ["1", "2", "3", "6"])
 def test_plan_ring_geometry_variants(orc, geom, monkeypatch):
     """KBMOD_STAGED_GEOM selects other slot sizes: the plan must stay exact and respect the cap."""
     monkeypatch.setenv("KBMOD_STAGED_GEOM", geom)
@@ -150,7 +150,7 @@ def test_plan_ring_geometry_variants(orc, geom, monkeypatch):
     st = synth.make_stack(cfg)
     pp = orc.make_psi_phi(st.sci, st.var, st.mask, st.psf)
     _, _, info = binding.debug_staged_plan(st.times, cfg.N, cfg.H, cfg.W, st.vel_grid)
-    assert info["CAP"] == {"1": 3072, "2": 6144, "3": 2560}[geom]
+    assert info["CAP"] == {"1": 3072, "2": 6144, "3": 2560, "6": 8192}[geom]
     check_against_oracle(orc, pp, st.times, st.vel_grid)
 
 
