@@ -261,3 +261,26 @@ def test_errors_are_loud(kb):
         kb.search(pp, [0.0, np.nan], np.zeros((1, 2), np.float32), 2, 1)      # bad time
     with pytest.raises(kb.KbmodError):
         kb.search(pp.cpu(), [0.0, 1.0], np.zeros((1, 2), np.float32), 2, 1)   # host tensor
+
+
+# ------------------------------------------------------------------------------ full size
+@pytest.mark.parametrize("which", [k for k in KERNELS if k != 1])
+def test_search_full_size_config3_sampled_bands(kb, orc, which):
+    """BASELINE.json configs[2] at full size, in the launch configuration bench.py times (GPU
+    psi/phi feeding the default search kernel): bands of start rows at the image edges, across
+    tile boundaries and in the interior are recomputed by the oracle on the same psi/phi and
+    must match bit for bit (every start pixel of the band, all K slots)."""
+    kb.set_search_kernel(which)
+    cfg = synth.config(3)
+    st = synth.make_stack(cfg)
+    pp = kb.make_psi_phi(_cuda(st.sci), _cuda(st.var), _cuda(st.mask), st.psf)
+    res = kb.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs)
+    pp_host = pp.cpu().numpy()
+    del pp
+    for y0 in (0, 28, 2044, cfg.H - 8):            # 8-row bands; 28..36 straddles a 30/32-row tile edge
+        ref = orc.search(pp_host, st.times, st.vel_grid, cfg.K, cfg.min_obs, y_begin=y0, y_end=y0 + 8)
+        gpu = {k: v[y0:y0 + 8].cpu().numpy() for k, v in res.items()}
+        assert_search_exact(gpu, ref)
+    # the injected sources are there: the best nu of the frame is a >= 8-observation detection
+    best = float(res["nu"][..., 0].max().item())
+    assert best > 10.0
