@@ -150,6 +150,10 @@ def run_reference(args, cfg, st):
     print(json.dumps(line))
 
 
+def evals_per_step(cfg, world):
+    return cfg.evals * world
+
+
 def config_dict(cfg, args):
     return {"workload": f"BASELINE.json configs[{args.config - 1}] {cfg.name}: N={cfg.N} "
                         f"{cfg.H}x{cfg.W} fp32, V={cfg.V} ({cfg.n_angles}x{cfg.n_speeds}), "
@@ -247,8 +251,31 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
 
     binding.search_status(ws)
     step_e2e()
-    e2e_ms = timed(step_e2e, max(1, min(args.steps, 5)))
     e2e_steps = max(1, min(args.steps, 5))
+    e2e_ms = timed(step_e2e, e2e_steps)
+
+    # the same step through the single C-ABI call that takes HOST buffers (kbmod_search_host);
+    # reported beside `e2e`, and only if its result planes equal the resident run's
+    host_abi = None
+    try:
+        if world > 1:
+            raise RuntimeError("measured at N=1 only")
+        ws_h = torch.empty(binding.search_host_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
+        run_h = lambda: binding.search_host(h_sci, h_var, h_mask, st.psf, st.times, st.vel_grid, K,
+                                            cfg.min_obs, h_out, ws_h)
+        run_h()
+        binding.search_status(ws_h)
+        same = all(torch.equal(h_out[k], out[k].cpu()) or k in ("nu", "alpha", "psi", "phi") and
+                   torch.equal(h_out[k].view(torch.int32), out[k].cpu().view(torch.int32)) for k in out)
+        if same:
+            ms = timed(run_h, e2e_steps) / e2e_steps
+            host_abi = {"value": evals_per_step(cfg, world) / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms,
+                        "call": "kbmod_search_host", "verified_equal_to_resident_run": True}
+        else:
+            host_abi = {"error": "result planes differ from the resident run"}
+        del ws_h
+    except Exception as exc:                                   # never costs the main line
+        host_abi = {"error": f"{type(exc).__name__}: {exc}"[:200]}
 
     if rank != 0:
         return
@@ -287,6 +314,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
                 "ms_per_step": e2e_ms / e2e_steps,
                 "h2d_bytes_per_step": int(h_sci.numel() * 4 + h_var.numel() * 4 + h_mask.numel()),
                 "d2h_bytes_per_step": int(sum(v.numel() * v.element_size() for v in h_out.values()))},
+        "e2e_host_abi": host_abi,
     }
     if world == 1 and not args.no_cpu:
         import oracle

@@ -126,6 +126,24 @@ int kbmod_search_split(const float* psi, const float* phi, const double* times, 
                        void* stream);
 
 /*
+ * The whole hot path from HOST buffers (S1..S6 plus the transfers): copies sci / var / mask to the
+ * device, runs kbmod_make_psi_phi and kbmod_search, and copies the six result planes back, all
+ * enqueued on `stream` (asynchronous with respect to the host when the host buffers are pinned;
+ * the call itself does not synchronise).  Same arithmetic and results as the two calls above.
+ *   sci, var : HOST [N][H][W] float;  mask : HOST [N][H][W] uint8 or NULL;  psf : HOST [N][P][P]
+ *   times    : HOST [N] double;       vel_grid : HOST [V][2] float
+ *   out      : HOST struct of HOST plane pointers, each [H][W][K]
+ *   workspace: DEVICE scratch of at least kbmod_search_host_workspace(N,H,W,V,K) bytes, 256-byte
+ *              aligned (holds the device copies of the inputs, psi/phi, the result planes and
+ *              the search workspace); kbmod_search_status(workspace, stream) works on it too
+ */
+int kbmod_search_host(const float* sci, const float* var, const uint8_t* mask, const float* psf,
+                      const double* times, int N, int H, int W, int P, const float* vel_grid, int V,
+                      int K, int min_obs, const kbmod_result* out, void* workspace,
+                      size_t workspace_bytes, void* stream);
+size_t kbmod_search_host_workspace(int N, int H, int W, int V, int K);
+
+/*
  * Test hook: evaluate an explicit list of M trajectories with exactly the arithmetic of
  * kbmod_search (S3 + S4), returning the coadds and every sampled pixel.
  *   x0y0 : [M][2] int32 device;  vxvy : [M][2] float device;  times : HOST [N] double

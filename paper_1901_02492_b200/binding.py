@@ -19,7 +19,8 @@ _lib: Optional[ctypes.CDLL] = None
 
 EXPORTS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_workspace", "kbmod_search_split",
            "kbmod_eval_trajectories", "kbmod_set_search_kernel", "kbmod_launch_count",
-           "kbmod_status_string", "kbmod_version", "kbmod_debug_staged_plan", "kbmod_search_status")
+           "kbmod_status_string", "kbmod_version", "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host",
+           "kbmod_search_host_workspace")
 
 
 class KbmodError(RuntimeError):
@@ -39,12 +40,14 @@ def lib() -> ctypes.CDLL:
                              "(or __graft_entry__.build()); there is no CPU fallback")
         L = ctypes.CDLL(LIB_PATH)
         L.kbmod_search_workspace.restype = ctypes.c_size_t
+        L.kbmod_search_host_workspace.restype = ctypes.c_size_t
         L.kbmod_launch_count.restype = ctypes.c_ulonglong
         L.kbmod_status_string.restype = ctypes.c_char_p
         L.kbmod_version.restype = ctypes.c_char_p
         for n in ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_split",
                   "kbmod_eval_trajectories", "kbmod_set_search_kernel",
-                  "kbmod_debug_staged_plan", "kbmod_search_status"):
+                  "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host",
+           "kbmod_search_host_workspace"):
             getattr(L, n).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -180,6 +183,42 @@ def search(psiphi: torch.Tensor, times, vel_grid, K: int, min_obs: int,
         # convenience path (no caller workspace to query later): wait and report a kernel that
         # gave up; callers that pass a workspace stay asynchronous and call search_status()
         search_status(workspace)
+    return out
+
+
+def search_host_workspace(N: int, H: int, W: int, V: int, K: int) -> int:
+    return int(lib().kbmod_search_host_workspace(N, H, W, V, K))
+
+
+def _hostbuf(t, dtype, what: str):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise KbmodError(f"{what}: expected a contiguous host tensor of {dtype} (pinned for async copies)")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def search_host(sci: torch.Tensor, var: torch.Tensor, mask: Optional[torch.Tensor], psf, times,
+                vel_grid, K: int, min_obs: int, out: Dict[str, torch.Tensor],
+                workspace: torch.Tensor) -> Dict[str, torch.Tensor]:
+    """kbmod_search_host: the whole hot path from HOST tensors (pinned for asynchronous copies) to
+    HOST result planes `out`; `workspace` is a CUDA uint8 tensor of search_host_workspace() bytes.
+    Enqueued on the current stream; synchronise it (or call search_status) before reading `out`."""
+    N, H, W = sci.shape
+    psf = _host(psf, np.float32)
+    times = _host(times, np.float64)
+    vel = _host(vel_grid, np.float32)
+    if psf.ndim != 3 or psf.shape[0] != N or psf.shape[1] != psf.shape[2]:
+        raise KbmodError("psf must be [N,P,P]")
+    res = _Result(*[_hostbuf(out[k], torch.int32 if k in ("vel_idx", "n_obs") else torch.float32, k)
+                    for k in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")])
+    rc = lib().kbmod_search_host(_hostbuf(sci, torch.float32, "sci"), _hostbuf(var, torch.float32, "var"),
+                                 _hostbuf(mask, torch.uint8, "mask"), psf.ctypes.data_as(ctypes.c_void_p),
+                                 times.ctypes.data_as(ctypes.c_void_p), N, H, W, int(psf.shape[1]),
+                                 vel.ctypes.data_as(ctypes.c_void_p), int(vel.shape[0]), int(K), int(min_obs),
+                                 ctypes.byref(res), _dev(workspace, torch.uint8, "workspace"),
+                                 ctypes.c_size_t(workspace.numel()), _stream())
+    _check(rc, "kbmod_search_host")
     return out
 
 

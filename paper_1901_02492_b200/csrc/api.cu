@@ -133,6 +133,74 @@ int kbmod_search_status(const void* workspace, void* stream) {
     return status == 0 ? KBMOD_OK : KBMOD_ERR_TIMEOUT;
 }
 
+namespace kbmod {
+struct HostLayout {
+    size_t search_off, sci_off, var_off, mask_off, pp_off, plane_off[6], total;
+};
+static HostLayout host_layout(int N, int H, int W, int V, int K) {
+    HostLayout l;
+    const size_t px = (size_t)N * H * W, rk = (size_t)H * W * K;
+    size_t off = 0;
+    l.search_off = off;                       // first: kbmod_search_status reads word 0 of the workspace
+    off = align_up(off + workspace_layout(N, H, W, V, K).total, 256);
+    l.sci_off = off; off = align_up(off + px * 4, 256);
+    l.var_off = off; off = align_up(off + px * 4, 256);
+    l.mask_off = off; off = align_up(off + px, 256);
+    l.pp_off = off; off = align_up(off + px * 8, 256);
+    for (int k = 0; k < 6; ++k) { l.plane_off[k] = off; off = align_up(off + rk * 4, 256); }
+    l.total = off;
+    return l;
+}
+}  // namespace kbmod
+
+size_t kbmod_search_host_workspace(int N, int H, int W, int V, int K) {
+    if (N <= 0 || H <= 0 || W <= 0 || V <= 0 || K <= 0) return 0;
+    return host_layout(N, H, W, V, K).total;
+}
+
+int kbmod_search_host(const float* sci, const float* var, const uint8_t* mask, const float* psf,
+                      const double* times, int N, int H, int W, int P, const float* vel_grid, int V,
+                      int K, int min_obs, const kbmod_result* out, void* workspace,
+                      size_t workspace_bytes, void* stream) {
+    if (!sci || !var || !psf || !times || !vel_grid || !out || !workspace) return KBMOD_ERR_NULL;
+    if (!out->vel_idx || !out->n_obs || !out->psi || !out->phi || !out->nu || !out->alpha)
+        return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0 || V <= 0 || K <= 0) return KBMOD_ERR_SHAPE;
+    if ((uintptr_t)workspace & 255) return KBMOD_ERR_ALIGN;
+    const HostLayout l = host_layout(N, H, W, V, K);
+    if (workspace_bytes < l.total) return KBMOD_ERR_WORKSPACE;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    char* ws = static_cast<char*>(workspace);
+    const size_t px = (size_t)N * H * W, rk = (size_t)H * W * K;
+    float* d_sci = reinterpret_cast<float*>(ws + l.sci_off);
+    float* d_var = reinterpret_cast<float*>(ws + l.var_off);
+    uint8_t* d_mask = mask ? reinterpret_cast<uint8_t*>(ws + l.mask_off) : nullptr;
+    float* d_pp = reinterpret_cast<float*>(ws + l.pp_off);
+    if (cudaMemcpyAsync(d_sci, sci, px * 4, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(d_var, var, px * 4, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        (mask && cudaMemcpyAsync(d_mask, mask, px, cudaMemcpyHostToDevice, st) != cudaSuccess))
+        return KBMOD_ERR_CUDA;
+    if (int rc = kbmod_make_psi_phi(d_sci, d_var, d_mask, psf, N, H, W, P, d_pp, stream)) return rc;
+    kbmod_result dev;
+    void* host_planes[6] = {out->vel_idx, out->n_obs, out->psi, out->phi, out->nu, out->alpha};
+    void* dev_planes[6];
+    for (int k = 0; k < 6; ++k) dev_planes[k] = ws + l.plane_off[k];
+    dev.vel_idx = static_cast<int32_t*>(dev_planes[0]);
+    dev.n_obs = static_cast<int32_t*>(dev_planes[1]);
+    dev.psi = static_cast<float*>(dev_planes[2]);
+    dev.phi = static_cast<float*>(dev_planes[3]);
+    dev.nu = static_cast<float*>(dev_planes[4]);
+    dev.alpha = static_cast<float*>(dev_planes[5]);
+    if (int rc = kbmod_search(d_pp, times, N, H, W, vel_grid, V, K, min_obs, &dev, ws + l.search_off,
+                              workspace_layout(N, H, W, V, K).total, stream))
+        return rc;
+    for (int k = 0; k < 6; ++k)
+        if (cudaMemcpyAsync(host_planes[k], dev_planes[k], rk * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+            return KBMOD_ERR_CUDA;
+    return KBMOD_OK;
+}
+
 int kbmod_search_split(const float* psi, const float* phi, const double* times, int N, int H,
                        int W, const float* vel_grid, int V, int K, int min_obs,
                        const kbmod_result* out, void* workspace, size_t workspace_bytes,

@@ -253,6 +253,23 @@ def test_search_split_entry_point(kb, orc):
     assert_search_exact(g, orc.search(pp, times, vel, 4, 2))
 
 
+def test_search_host_entry_point(kb, orc):
+    """kbmod_search_host (HOST buffers in, HOST planes out) equals the two device-pointer calls."""
+    cfg = synth.config(2, N=8, H=75, W=203)
+    st = synth.make_stack(cfg)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    out = {k: torch.empty((cfg.H, cfg.W, cfg.K), dtype=torch.int32 if k in ("vel_idx", "n_obs") else torch.float32).pin_memory()
+           for k in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")}
+    ws = torch.empty(kb.search_host_workspace(cfg.N, cfg.H, cfg.W, cfg.V, cfg.K), dtype=torch.uint8, device="cuda")
+    kb.search_host(pin(st.sci), pin(st.var), pin(st.mask), st.psf, st.times, st.vel_grid, cfg.K, cfg.min_obs, out, ws)
+    kb.search_status(ws)                                  # synchronises
+    pp = kb.make_psi_phi(_cuda(st.sci), _cuda(st.var), _cuda(st.mask), st.psf)
+    ref = _np(kb.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs))
+    assert_search_exact({k: v.numpy() for k, v in out.items()}, ref)
+    # and the oracle agrees on the same psi/phi
+    assert_search_exact(ref, orc.search(pp.cpu().numpy(), st.times, st.vel_grid, cfg.K, cfg.min_obs))
+
+
 def test_errors_are_loud(kb):
     pp = _cuda(synth.random_psiphi(2, 8, 8, seed=1))
     with pytest.raises(kb.KbmodError):
