@@ -183,6 +183,21 @@ def test_search_slow_velocities_interior(kb, orc, which):
 
 
 @pytest.mark.parametrize("which", KERNELS)
+def test_search_maximum_image_count(kb, orc, which):
+    """N = KBMOD_MAX_IMAGES = 64 (and N = 40, the largest stack of BASELINE.json configs[4])."""
+    kb.set_search_kernel(which)
+    rng = np.random.default_rng(64)
+    for N, mo in ((64, 20), (40, 20)):
+        pp = synth.random_psiphi(N, 40, 70, seed=N, invalid_frac=0.05)
+        times = np.sort(rng.uniform(0.0, 5.0, N))
+        vel = synth.velocity_grid(6, 4, -math.pi / 2, math.pi / 2, 1.0, 9.0)
+        gpu = _np(kb.search(_cuda(pp), times, vel, 8, mo))
+        assert_search_exact(gpu, orc.search(pp, times, vel, 8, mo))
+    with pytest.raises(kb.KbmodError):                                        # N = 65: beyond the limit
+        kb.search(_cuda(synth.random_psiphi(65, 4, 4, seed=1)), np.arange(65.0), vel, 2, 1)
+
+
+@pytest.mark.parametrize("which", KERNELS)
 def test_search_edge_cases(kb, orc, which):
     kb.set_search_kernel(which)
     rng = np.random.default_rng(4)

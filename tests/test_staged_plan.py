@@ -190,3 +190,13 @@ def test_plan_degenerate_shapes(orc):
     vel = np.concatenate([vel, vel[3:9], vel[:2], np.array([[5e4, 0], [0, -7e4], [3e3, 3e3]], np.float32)])
     times = np.array([5.0, 4.5, 6.0, 5.25, 7.0])
     check_against_oracle(orc, pp, times, vel)
+
+
+def test_plan_maximum_image_count(orc):
+    """N = 64 = KBMOD_MAX_IMAGES and N = 40 (the additive-count variants of the kernel)."""
+    rng = np.random.default_rng(64)
+    for N in (64, 40):
+        pp = synth.random_psiphi(N, 40, 70, seed=N, invalid_frac=0.05)
+        times = np.sort(rng.uniform(0.0, 5.0, N))
+        vel = synth.velocity_grid(6, 4, -math.pi / 2, math.pi / 2, 1.0, 9.0)
+        check_against_oracle(orc, pp, times, vel)
