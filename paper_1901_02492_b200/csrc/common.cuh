@@ -5,6 +5,14 @@
 #include <stddef.h>
 #include "kbmod_b200.h"
 
+// Kernel launch.  The SIMT-emulation test build (tests/hostlogic/simt/, g++, no GPU) runs the
+// kernel's CTAs on the CPU instead; the product build is the plain triple-chevron launch.
+#if defined(KBMOD_SIMT_EMUL)
+#define KBMOD_LAUNCH(kern, grid, block, smem, stream, ...) ::simt::launch(kern, (unsigned)(grid), (unsigned)(block), (size_t)(smem), __VA_ARGS__)
+#else
+#define KBMOD_LAUNCH(kern, grid, block, smem, stream, ...) kern<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__)
+#endif
+
 namespace kbmod {
 
 // every kernel launch of the library goes through this counter (kbmod_launch_count()).

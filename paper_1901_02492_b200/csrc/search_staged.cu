@@ -357,9 +357,18 @@ encode_kernel(const float2* __restrict__ in, float4* __restrict__ out, int W, in
     }
 }
 
+// The inline-PTX helpers.  tests/test_staged_simt.py compiles this file with g++ against a SIMT
+// emulator (tests/hostlogic/simt/) and defines KBMOD_SIMT_EMUL as the header that supplies host
+// stand-ins of the same names; the product build never defines it.
+#if defined(KBMOD_SIMT_EMUL)
+#include KBMOD_SIMT_EMUL
+#else
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
 __device__ __forceinline__ void mbar_arrive(unsigned bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
@@ -376,21 +385,6 @@ __device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
         "selp.u32 %0, 1, 0, p;\n"
         "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
-}
-// Warp-uniform bounded wait (all 32 lanes must call it).  A wait that lasts WAIT_LIMIT_CLOCKS
-// (about two seconds; a healthy wait is microseconds) means the pipeline is broken: the warp
-// gives up instead of hanging the GPU, and the caller reports KBMOD_ERR_TIMEOUT.
-constexpr long long WAIT_LIMIT_CLOCKS = 1ll << 32;
-__device__ __forceinline__ bool mbar_wait(unsigned bar, unsigned parity) {
-    bool ok = mbar_try_wait(bar, parity);
-    if (!ok) {
-        const long long t0 = clock64();
-        for (;;) {
-            ok = mbar_try_wait(bar, parity);
-            if (ok || clock64() - t0 > WAIT_LIMIT_CLOCKS) break;
-        }
-    }
-    return __all_sync(0xFFFFFFFFu, ok);
 }
 __device__ __forceinline__ void tma_load_3d(unsigned dst, const void* tmap, int c0, int c1, int c2, unsigned bar) {
     asm volatile(
@@ -415,6 +409,23 @@ __device__ __forceinline__ int4 lds128(unsigned a) {
     int4 v;
     asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
     return v;
+}
+#endif  // KBMOD_SIMT_EMUL
+
+// Warp-uniform bounded wait (all 32 lanes must call it).  A wait that lasts WAIT_LIMIT_CLOCKS
+// (about two seconds; a healthy wait is microseconds) means the pipeline is broken: the warp
+// gives up instead of hanging the GPU, and the caller reports KBMOD_ERR_TIMEOUT.
+constexpr long long WAIT_LIMIT_CLOCKS = 1ll << 32;
+__device__ __forceinline__ bool mbar_wait(unsigned bar, unsigned parity) {
+    bool ok = mbar_try_wait(bar, parity);
+    if (!ok) {
+        const long long t0 = clock64();
+        for (;;) {
+            ok = mbar_try_wait(bar, parity);
+            if (ok || clock64() - t0 > WAIT_LIMIT_CLOCKS) break;
+        }
+    }
+    return __all_sync(0xFFFFFFFFu, ok);
 }
 __device__ __forceinline__ void acc_add(u64& a, u64 s) {      // (Psi, -Phi) += (psi, -phi), RN each
     float2 fa = make_float2(__uint_as_float((unsigned)a), __uint_as_float((unsigned)(a >> 32)));
@@ -520,7 +531,7 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
             mbar_init(bar_full + 8 * s, 1);
             mbar_init(bar_empty + 8 * s, NCW);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_mbar_init();
     }
     __syncthreads();
 
@@ -569,6 +580,11 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
                             ra.release_oldest();
                             if (++oslot == NSLOT) { oslot = 0; ophase ^= 1; }
                         }
+                        // adv[] is shared by the 32 lanes: when the header ring is the limit, place()
+                        // rewrites the very word release_oldest() has just read (next % NH == oldest %
+                        // NH), so no lane may place before every lane has released (found by the SIMT
+                        // emulation, tests/test_staged_simt.py: lanes are not in lockstep)
+                        __syncwarp();
                         const unsigned off = ra.place(need);
                         box_at = ring + off;
                         if (type == ENT_TMA && lane == 6) hv = (int)off;
@@ -580,7 +596,7 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
                         box_at = sa + HDR_BYTES;
                         if (type == ENT_TMA && lane == 6) hv = HDR_BYTES + (int)(slot * SLOT_BYTES);
                     }
-                    if (lane < HDR_INTS) asm volatile("st.shared.b32 [%0], %1;" ::"r"(sa + 4 * lane), "r"(hv) : "memory");
+                    if (lane < HDR_INTS) sts32(sa + 4 * lane, hv);
                     __syncwarp();
                     if (lane == 0) {
                         if (load) {
@@ -856,7 +872,7 @@ static int launch_variant(const StagedParams& prm, const StagedMaps& maps, int g
             return KBMOD_ERR_CUDA;
         attr_set = true;
     }
-    kern<<<grid, THREADS, smem_bytes_of(G), st>>>(prm, maps);
+    KBMOD_LAUNCH(kern, grid, THREADS, smem_bytes_of(G), st, prm, maps);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }
@@ -903,7 +919,7 @@ int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, 
 
     if (cudaMemsetAsync(status_dev, 0, sizeof(int), st) != cudaSuccess) return KBMOD_ERR_CUDA;
     const int Wp = (W + 1) & ~1;
-    encode_kernel<<<148 * 8, 256, 0, st>>>(psiphi, reinterpret_cast<float4*>(enc_dev), W, Wp, (size_t)N * H);
+    KBMOD_LAUNCH(encode_kernel, 148 * 8, 256, 0, st, psiphi, reinterpret_cast<float4*>(enc_dev), W, Wp, (size_t)N * H);
     note_launch();
     if (cudaGetLastError() != cudaSuccess) return KBMOD_ERR_CUDA;
 

@@ -1,0 +1,53 @@
+// tests/hostlogic/staged_simt.cpp -- TEST INFRASTRUCTURE.  Compiles csrc/search_staged.cu with g++
+// against the SIMT emulator of tests/hostlogic/simt/ and exposes launch_search_staged (host plan,
+// tensor maps, encode kernel, the persistent producer/consumer kernel) as a C function over HOST
+// memory, so that tests/test_staged_simt.py can compare the kernel's device-side logic with the
+// oracle without a GPU.  Built by the test with
+//   g++ -O1 -std=c++17 -ffp-contract=off -shared -fPIC -Itests/hostlogic/simt -Iinclude
+//       -Ipaper_1901_02492_b200/csrc -DKBMOD_SIMT_EMUL='"simt_ptx.h"' tests/hostlogic/staged_simt.cpp
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+namespace kbmod {
+alignas(1024) unsigned char smem_raw[simt::SMEM_MAX + 64];
+inline unsigned smem_u32(const void* p) {
+    return simt::SMEM_BASE + (unsigned)(static_cast<const unsigned char*>(p) - smem_raw);
+}
+}  // namespace kbmod
+
+#include "search_staged.cu"
+
+namespace kbmod {
+void note_launch(int) {}
+}  // namespace kbmod
+
+extern "C" {
+
+// stats[0..5] = shared-memory faults, TMA loads, TMA alignment faults, kernel launches, status word, plan entries
+int simt_search_staged(const float* psiphi, const double* times, int N, int H, int W, const float* vel_grid, int V,
+                       int K, int min_obs, int32_t* vel_idx, int32_t* n_obs, float* psi, float* phi, float* nu,
+                       float* alpha, int order, unsigned seed, int sms, int tma_delay, long long* stats) {
+    using namespace kbmod;
+    simt::cfg().order = order;
+    simt::cfg().seed = seed;
+    simt::cfg().sms = sms;
+    simt::cfg().tma_delay = tma_delay;
+    simt::State& s = simt::S();
+    s.smem = smem_raw;
+    s.smem_faults = s.tma_loads = s.tma_faults = s.launches = 0;
+    DtTable dt;
+    for (int i = 0; i < KBMOD_MAX_IMAGES; ++i) dt.dt[i] = 0.0f;
+    for (int i = 0; i < N; ++i) dt.dt[i] = (float)(times[i] - times[0]);
+    kbmod_result out{vel_idx, n_obs, psi, phi, nu, alpha};
+    std::vector<unsigned char> plan(staged_plan_bytes(N, V) + 256), enc(staged_enc_bytes(N, H, W) + 256);
+    unsigned char* encp = enc.data() + ((256 - ((uintptr_t)enc.data() & 255)) & 255);
+    int status = 0;
+    const int rc = launch_search_staged(reinterpret_cast<const float2*>(psiphi), dt, N, H, W, vel_grid, V, K, min_obs,
+                                        out, plan.data(), reinterpret_cast<const float2*>(vel_grid),
+                                        reinterpret_cast<float2*>(encp), &status, nullptr);
+    stats[0] = s.smem_faults; stats[1] = s.tma_loads; stats[2] = s.tma_faults; stats[3] = s.launches;
+    stats[4] = status; stats[5] = 0;
+    return rc;
+}
+
+}  // extern "C"
