@@ -157,8 +157,10 @@ int kbmod_eval_trajectories(const float* psiphi, const double* times, int N, int
 
 /* Selects the search kernel: 0 = automatic (default: the tiled kernel where the shape fits, else
  * the direct-gather kernel), 1 = direct-gather kernel (global loads, any shape), 2 = tiled kernel
- * (host-proven integer shifts, global loads through L1), 3 = TMA-staged shared-memory kernel.
- * With 2 or 3 kbmod_search returns KBMOD_ERR_UNSUPPORTED if the shape does not fit that kernel.
+ * (host-proven integer shifts, global loads through L1), 3 = TMA-staged shared-memory kernel,
+ * 4 = tiled kernel with queue-compacted top-K (the gathers of 2, the S5/S6 of 3).
+ * With 2, 3 or 4 kbmod_search returns KBMOD_ERR_UNSUPPORTED if the shape does not fit that kernel.
+ * All kernels return bit-identical results.
  * Process-wide; for tests and benchmarks. */
 int kbmod_set_search_kernel(int which);
 

@@ -74,7 +74,7 @@ size_t kbmod_search_workspace(int N, int H, int W, int V, int K) {
 }
 
 int kbmod_set_search_kernel(int which) {
-    if (which < 0 || which > 3) return KBMOD_ERR_ARG;
+    if (which < 0 || which > 4) return KBMOD_ERR_ARG;
     g_search_kernel.store(which);
     return KBMOD_OK;
 }
@@ -116,8 +116,8 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
     if (which != 1) {
         const int rc = launch_search_tiled(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out,
                                            ws + l.plan_off, vel_dev,
-                                           reinterpret_cast<float2*>(ws + l.enc_off), st);
-        if (rc != KBMOD_ERR_UNSUPPORTED || which == 2) return rc;
+                                           reinterpret_cast<float2*>(ws + l.enc_off), which == 4, st);
+        if (rc != KBMOD_ERR_UNSUPPORTED || which == 2 || which == 4) return rc;
     }
     return launch_search_direct(pp, dt, N, H, W, vel_dev, V, K, min_obs, *out, st);
 }

@@ -28,6 +28,7 @@
 #include <vector>
 
 #include "search_tiled.cuh"
+#include "topk_list.h"
 
 namespace kbmod {
 
@@ -179,7 +180,13 @@ encode_kernel(const float4* __restrict__ in, float4* __restrict__ out, size_t n2
 typedef unsigned long long u64;
 
 __device__ __forceinline__ void acc_add(u64& a, u64 s) {      // (Psi, -Phi) += (psi, -phi), RN each
+#if defined(KBMOD_SIMT_EMUL)      // host build of the SIMT-emulation tests: two plain binary32 adds
+    const float x = __fadd_rn(__uint_as_float((unsigned)a), __uint_as_float((unsigned)s));
+    const float y = __fadd_rn(__uint_as_float((unsigned)(a >> 32)), __uint_as_float((unsigned)(s >> 32)));
+    a = (u64)__float_as_uint(x) | ((u64)__float_as_uint(y) << 32);
+#else
     asm("add.rn.f32x2 %0, %0, %1;" : "+l"(a) : "l"(s));
+#endif
 }
 __device__ __forceinline__ u64 ld_sample(const u64* p) { return __ldg(p); }
 
@@ -439,6 +446,302 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// Kernel 4: the same gathers, S5/S6 off the common path (queue-compacted top-K)
+// ---------------------------------------------------------------------------------------------
+// search_tiled_kernel spends three quarters of its instructions in the shared-memory list code,
+// because a warp enters it whenever ANY of its 32 lanes passes the pre-test (ncu, profiles/
+// r01_v2_tiled.md).  Here the survivors of the pre-test are compacted by ballot into a per-warp
+// shared-memory queue and handled 32 at a time, one lane per candidate: correctly rounded
+// score, sorted insert into the pixel's list.  The lists live in the nu / vel_idx output planes
+// (only the owning warp touches a pixel's list, through L2), so shared memory holds only the
+// block record and the queues.  S5/S6 are the code of the staged kernel (search_staged.cu),
+// whose logic tests/test_staged_simt.py checks on the CPU; S3/S4 are search_tiled_kernel's.
+constexpr int QCAP = 64;                  // per-warp candidate queue entries (power of two, >= 63)
+
+struct ListMemPlanes {                    // list entries are read and written through L2
+    template <class T> static __device__ __forceinline__ T ld(const T* p) { return __ldcg(p); }
+    template <class T> static __device__ __forceinline__ void st(T* p, T v) { __stcg(p, v); }
+};
+
+// One dense pass over up to 32 queued candidates of this warp: lane l takes entry qhead + l.
+template <int RX, int KP>
+__device__ __forceinline__ void process_batch_q(const TiledParams& prm, const float* q_psi, const float* q_phi,
+                                                const unsigned* q_meta, unsigned qhead, int n, int lane,
+                                                int wx0, int wy0) {
+    bool valid = lane < n;
+    const unsigned idx = (qhead + lane) & (QCAP - 1);
+    const float Psi = q_psi[idx], Phi = q_phi[idx];
+    const unsigned meta = q_meta[idx];
+    const int pix = meta & 127, j = (int)(meta >> 7);
+    const int r = pix >> 5, ln = pix & 31;
+    const int x = wx0 + ln + 32 * (r % RX), y = wy0 + r / RX;
+    const float nu = valid ? score_nu(Psi, Phi) : 0.0f;
+    const size_t p = valid ? ((size_t)y * prm.W + x) * prm.K : 0;
+    for (;;) {
+        // two candidates of the same pixel in one batch: lowest lane first, the rest next round
+        const unsigned same = __match_any_sync(0xFFFFFFFFu, valid ? pix : 128 + lane);
+        if (valid && lane == __ffs(same) - 1) {
+            list_insert<KP, ListMemPlanes>(prm.out.nu + p, prm.out.vel_idx + p, prm.K, nu, j);
+            valid = false;
+        }
+        __syncwarp();
+        if (!__any_sync(0xFFFFFFFFu, valid)) break;
+    }
+}
+
+// RX x RY pixels per thread: x = tile_x + rx * 32 + lane, y = tile_y + warp * RY + ry; B * RX * RY = 32
+template <int RX, int RY, int B, int KP>
+__global__ void __launch_bounds__(THREADS, 1)
+search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
+    constexpr int R = RX * RY;
+    static_assert(B * R == 32, "the scoring switch lists B*R = 32 steps");
+    constexpr int TW = 32 * RX, TH = RY * (THREADS / 32);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = prm.N, H = prm.H, W = prm.W, K = prm.K;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int rec_n = (int)rec_ints(B, N);
+    int* rec = reinterpret_cast<int*>(smem_raw);                  // off[B][N], sh[B][N], meta[B][META]
+    float* q_psi = reinterpret_cast<float*>(rec + rec_n) + warp * (3 * QCAP);
+    float* q_phi = q_psi + QCAP;
+    unsigned* q_meta = reinterpret_cast<unsigned*>(q_phi + QCAP);
+
+    int tx, ty;                                                   // tile order: see search_tiled_kernel
+    {
+        const int per_group = prm.group_w * prm.tiles_y;
+        const int g = blockIdx.x / per_group, rem = blockIdx.x - g * per_group;
+        const int gw = min(prm.group_w, prm.tiles_x - g * prm.group_w);
+        ty = rem / gw;
+        tx = g * prm.group_w + (rem - ty * gw);
+    }
+    const int tile_x = tx * TW, tile_y = ty * TH;
+    const int x_first = tile_x + lane;
+    const int y_first = tile_y + warp * RY;
+    const bool ragged = (tile_x + TW > W) || (tile_y + TH > H);
+    const int tile_x1 = min(tile_x + TW, W) - 1, tile_y1 = min(tile_y + TH, H) - 1;
+    unsigned inimg = 0;                                           // bit r: pixel r of this thread is inside the image
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+        inimg |= ((x_first + 32 * (r % RX) < W) && (y_first + r / RX < H)) ? (1u << r) : 0u;
+    const size_t pix0 = (size_t)y_first * W + x_first;            // pixel r: pix0 + 32*rx + ry*W
+
+    const u64* basep[RY];
+#pragma unroll
+    for (int ry = 0; ry < RY; ++ry)
+        basep[ry] = prm.enc + (size_t)min(y_first + ry, H - 1) * W + min(x_first, W - 1);
+
+    // empty lists (in the output planes)
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+        if (inimg & (1u << r)) {
+            const size_t p = (pix0 + 32 * (r % RX) + (size_t)(r / RX) * W) * K;
+            for (int kk = 0; kk < K; ++kk) {
+                __stcg(prm.out.nu + p + kk, -INFINITY);
+                __stcg(prm.out.vel_idx + p + kk, LIST_EMPTY_IDX);
+            }
+        }
+    __syncwarp();
+    unsigned qhead = 0, qtail = 0;
+    const unsigned minobs = (unsigned)prm.min_obs;
+
+    int* r_off = rec;
+    int* r_sh = rec + B * N;
+    int* r_meta = rec + 2 * B * N;
+
+    for (int blk = 0; blk < prm.nblk; ++blk) {
+        __syncthreads();
+        {
+            const int* src = prm.plan + (size_t)blk * rec_n;
+            for (int k = tid; k < rec_n; k += THREADS) rec[k] = __ldg(src + k);
+        }
+        __syncthreads();
+
+        float lo[R];                               // pre-test bound: K-th best nu minus a safety margin
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            float w = -INFINITY;
+            if (inimg & (1u << r))
+                w = __ldcg(prm.out.nu + (pix0 + 32 * (r % RX) + (size_t)(r / RX) * W) * K + (K - 1));
+            lo[r] = fmaf(-fabsf(w), 4e-6f, w);                   // -inf stays -inf
+        }
+
+        u64 acc[B][R];
+        unsigned cnt[B][R];
+        unsigned fast = 0;          // bit b: every window of velocity b is inside the image
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                // image 0 has dt = 0: shift (0,0) for every velocity
+                const u64 s0 = (inimg & (1u << r)) ? ld_sample(basep[r / RX] + 32 * (r % RX)) : 0ull;
+                acc[b][r] = s0;
+                cnt[b][r] = (unsigned)(s0 >> 63);
+            }
+            const int bx = r_meta[b * META + 1], by = r_meta[b * META + 2];
+            const int sxlo = (short)(bx & 0xFFFF), sxhi = bx >> 16;
+            const int sylo = (short)(by & 0xFFFF), syhi = by >> 16;
+            const bool ok = r_meta[b * META + 3] && !ragged && tile_x + sxlo >= 0 &&
+                            tile_x1 + sxhi < W && tile_y + sylo >= 0 && tile_y1 + syhi < H;
+            fast |= ok ? (1u << b) : 0u;
+        }
+
+        for (int i = 1; i < N; ++i) {
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                if (fast & (1u << b)) {
+                    const int o = r_off[b * N + i];
+#pragma unroll
+                    for (int ry = 0; ry < RY; ++ry) {
+                        const u64* p = basep[ry] + o;
+#pragma unroll
+                        for (int rx = 0; rx < RX; ++rx) {
+                            const u64 s = ld_sample(p + 32 * rx);
+                            acc_add(acc[b][ry * RX + rx], s);
+                            cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
+                        }
+                    }
+                } else {
+                    const int code = r_sh[b * N + i];
+                    if (code == SH_SKIP) continue;
+                    const u64* img = prm.enc + (size_t)i * H * W;
+                    if (code != SH_UNSAFE) {
+                        const int sx = (short)(code & 0xFFFF), sy = code >> 16;
+                        // whole window outside: nothing to add (uniform over the CTA)
+                        if (tile_x1 + sx < 0 || tile_x + sx >= W || tile_y1 + sy < 0 || tile_y + sy >= H)
+                            continue;
+#pragma unroll
+                        for (int ry = 0; ry < RY; ++ry) {
+                            const int y = y_first + ry + sy;
+                            const bool yin = (y_first + ry < H) && y >= 0 && y < H;
+#pragma unroll
+                            for (int rx = 0; rx < RX; ++rx) {
+                                const int x = x_first + 32 * rx + sx;
+                                const bool in = yin && (x_first + 32 * rx < W) && x >= 0 && x < W;
+                                const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
+                                acc_add(acc[b][ry * RX + rx], s);
+                                cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
+                            }
+                        }
+                    } else {
+                        const float vx = __int_as_float(r_meta[b * META + 4]);
+                        const float vy = __int_as_float(r_meta[b * META + 5]);
+                        const float dti = prm.dt.dt[i];
+#pragma unroll
+                        for (int ry = 0; ry < RY; ++ry) {
+                            int y = 0;
+                            const bool yin = traj_pixel(y_first + ry, vy, dti, H, y) && (y_first + ry < H);
+#pragma unroll
+                            for (int rx = 0; rx < RX; ++rx) {
+                                int x = 0;
+                                const bool in = traj_pixel(x_first + 32 * rx, vx, dti, W, x) && yin &&
+                                                (x_first + 32 * rx < W);
+                                const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
+                                acc_add(acc[b][ry * RX + rx], s);
+                                cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+
+        // ---- S5 + S6 for the B x R trajectories of this block.  The steps are the cases of one
+        // switch so that a single copy of the batch code serves all of them: a step that fills the
+        // queue to 32 leaves the switch, the batch is processed, and the switch is re-entered at
+        // the next step.
+        int step = 0;
+        for (;;) {
+            bool flush = false;
+            switch (step) {
+#define KBMOD_SCORE_STEP(S)                                                                              \
+    case S: {                                                                                            \
+        constexpr int b_ = (S) / R, r_ = (S) % R;                                                        \
+        const int j = r_meta[b_ * META + 0];                                                             \
+        if (j >= 0) {                                                                                    \
+            const float Psi = __uint_as_float((unsigned)acc[b_][r_]);                                    \
+            const float Phi = 0.0f - __uint_as_float((unsigned)(acc[b_][r_] >> 32));                     \
+            const bool pass = (cnt[b_][r_] >= minobs) && (Phi > 0.0f) && ((inimg >> r_) & 1u) &&         \
+                              !(Psi * rsqrtf(Phi) < lo[r_]);                                             \
+            const unsigned m = __ballot_sync(0xFFFFFFFFu, pass);                                         \
+            if (m) {                                                                                     \
+                if (pass) {                                                                              \
+                    const unsigned qi = (qtail + __popc(m & ((1u << lane) - 1u))) & (QCAP - 1);          \
+                    q_psi[qi] = Psi;                                                                     \
+                    q_phi[qi] = Phi;                                                                     \
+                    q_meta[qi] = ((unsigned)j << 7) | (r_ << 5) | lane;                                  \
+                }                                                                                        \
+                qtail += __popc(m);                                                                      \
+                if (qtail - qhead >= 32) {                                                               \
+                    step = (S) + 1;                                                                      \
+                    flush = true;                                                                        \
+                    break;                                                                               \
+                }                                                                                        \
+            }                                                                                            \
+        }                                                                                                \
+    }
+                KBMOD_SCORE_STEP(0) KBMOD_SCORE_STEP(1) KBMOD_SCORE_STEP(2) KBMOD_SCORE_STEP(3)
+                KBMOD_SCORE_STEP(4) KBMOD_SCORE_STEP(5) KBMOD_SCORE_STEP(6) KBMOD_SCORE_STEP(7)
+                KBMOD_SCORE_STEP(8) KBMOD_SCORE_STEP(9) KBMOD_SCORE_STEP(10) KBMOD_SCORE_STEP(11)
+                KBMOD_SCORE_STEP(12) KBMOD_SCORE_STEP(13) KBMOD_SCORE_STEP(14) KBMOD_SCORE_STEP(15)
+                KBMOD_SCORE_STEP(16) KBMOD_SCORE_STEP(17) KBMOD_SCORE_STEP(18) KBMOD_SCORE_STEP(19)
+                KBMOD_SCORE_STEP(20) KBMOD_SCORE_STEP(21) KBMOD_SCORE_STEP(22) KBMOD_SCORE_STEP(23)
+                KBMOD_SCORE_STEP(24) KBMOD_SCORE_STEP(25) KBMOD_SCORE_STEP(26) KBMOD_SCORE_STEP(27)
+                KBMOD_SCORE_STEP(28) KBMOD_SCORE_STEP(29) KBMOD_SCORE_STEP(30) KBMOD_SCORE_STEP(31)
+#undef KBMOD_SCORE_STEP
+                default: break;
+            }
+            if (!flush) break;
+            __syncwarp();
+            process_batch_q<RX, KP>(prm, q_psi, q_phi, q_meta, qhead, 32, lane, tile_x, y_first);
+            qhead += 32;
+        }
+        __syncwarp();
+    }
+
+    // ---- end of tile: drain the queue, then re-evaluate the winners literally and write them
+    __syncwarp();
+    while (qtail != qhead) {
+        const int n = (int)min(32u, qtail - qhead);
+        process_batch_q<RX, KP>(prm, q_psi, q_phi, q_meta, qhead, n, lane, tile_x, y_first);
+        qhead += n;
+    }
+    __syncwarp();
+#pragma unroll 1
+    for (int r = 0; r < R; ++r) {
+        if (!(inimg & (1u << r))) continue;
+        const int x0 = x_first + 32 * (r % RX), y0 = y_first + r / RX;
+        const size_t obase = ((size_t)y0 * W + x0) * K;
+        for (int k = 0; k < K; ++k) {
+            const int bj = __ldcg(prm.out.vel_idx + obase + k);
+            if (bj != LIST_EMPTY_IDX) {
+                // literal evaluation (bit-identical sums: same samples, same order)
+                float Psi = 0.0f, Phi = 0.0f;
+                int n = 0;
+                const float2 v = __ldg(prm.vel + bj);
+                for (int i = 0; i < N; ++i) {
+                    int ix, iy;
+                    if (traj_pixel(x0, v.x, prm.dt.dt[i], W, ix) && traj_pixel(y0, v.y, prm.dt.dt[i], H, iy)) {
+                        const float2 s = __ldg(prm.psiphi + ((size_t)i * H + iy) * W + ix);
+                        if (s.x == s.x) { Psi = __fadd_rn(Psi, s.x); Phi = __fadd_rn(Phi, s.y); ++n; }
+                    }
+                }
+                prm.out.n_obs[obase + k] = n;
+                prm.out.psi[obase + k] = Psi;
+                prm.out.phi[obase + k] = Phi;
+                prm.out.nu[obase + k] = score_nu(Psi, Phi);
+                prm.out.alpha[obase + k] = score_alpha(Psi, Phi);
+            } else {
+                prm.out.vel_idx[obase + k] = -1;
+                prm.out.n_obs[obase + k] = 0;
+                prm.out.psi[obase + k] = 0.0f;
+                prm.out.phi[obase + k] = 0.0f;
+                prm.out.nu[obase + k] = -INFINITY;
+                prm.out.alpha[obase + k] = 0.0f;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // launch
 // ---------------------------------------------------------------------------------------------
 template <int RX, int RY, int WX, int B, int KMAX>
@@ -458,16 +761,39 @@ static int launch_variant(TiledParams& prm, cudaStream_t st) {
     prm.group_w = std::max(1, 512 / G::TW);
     const long long tiles = (long long)prm.tiles_x * prm.tiles_y;
     if (tiles > 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
-    kern<<<(unsigned)tiles, THREADS, smem, st>>>(prm);
+    KBMOD_LAUNCH(kern, (unsigned)tiles, THREADS, smem, st, prm);
+    note_launch();
+    return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
+}
+
+template <int RX, int RY, int B, int KP>
+static int launch_variant_q(TiledParams& prm, cudaStream_t st) {
+    constexpr int TW = 32 * RX, TH = RY * (THREADS / 32);
+    const size_t smem = rec_ints(B, prm.N) * sizeof(int) + (size_t)(THREADS / 32) * QCAP * 12;
+    if (smem > 227 * 1024) return KBMOD_ERR_UNSUPPORTED;
+    auto kern = search_tiledq_kernel<RX, RY, B, KP>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess)
+            return KBMOD_ERR_CUDA;
+        attr_set = true;
+    }
+    prm.tiles_x = (prm.W + TW - 1) / TW;
+    prm.tiles_y = (prm.H + TH - 1) / TH;
+    prm.group_w = std::max(1, 512 / TW);
+    const long long tiles = (long long)prm.tiles_x * prm.tiles_y;
+    if (tiles > 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
+    KBMOD_LAUNCH(kern, (unsigned)tiles, THREADS, smem, st, prm);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }
 
 int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, int W,
                         const float* vel_host, int V, int K, int min_obs, const kbmod_result& out,
-                        void* plan_dev, const float2* vel_dev, float2* enc_dev, cudaStream_t st) {
+                        void* plan_dev, const float2* vel_dev, float2* enc_dev, bool queued, cudaStream_t st) {
     // limits of the int16 shift encoding and of the int32 element offsets
     if (W > 30000 || H > 30000) return KBMOD_ERR_UNSUPPORTED;
+    if (queued && V >= (1 << 24)) return KBMOD_ERR_UNSUPPORTED;    // 25-bit velocity index in the queue word
     if ((long long)(N + 1) * H * W + (long long)SH_LIMIT * (W + 1) >= 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
     const int B = block_size_for_k(K);
     std::vector<int> plan;
@@ -476,8 +802,8 @@ int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, i
         return KBMOD_ERR_CUDA;
 
     const size_t n = (size_t)N * H * W;
-    encode_kernel<<<148 * 8, 256, 0, st>>>(reinterpret_cast<const float4*>(psiphi),
-                                          reinterpret_cast<float4*>(enc_dev), n / 2, psiphi, enc_dev, n);
+    KBMOD_LAUNCH(encode_kernel, 148 * 8, 256, 0, st, reinterpret_cast<const float4*>(psiphi),
+                 reinterpret_cast<float4*>(enc_dev), n / 2, psiphi, enc_dev, n);
     note_launch();
     if (cudaGetLastError() != cudaSuccess) return KBMOD_ERR_CUDA;
 
@@ -489,6 +815,11 @@ int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, i
     prm.nblk = nblk; prm.N = N; prm.H = H; prm.W = W; prm.K = K; prm.min_obs = min_obs;
     prm.out = out;
     prm.dt = dt;
+    if (queued) {                                                   // kernel 4: same tiles, queue-compacted S5/S6
+        if (K <= 8) return launch_variant_q<2, 2, 8, 8>(prm, st);
+        if (K <= 16) return launch_variant_q<2, 1, 16, 0>(prm, st);
+        return launch_variant_q<1, 1, 32, 0>(prm, st);
+    }
     if (K <= 8) return launch_variant<2, 2, 1, 8, 8>(prm, st);      // tile 64 x 32
     if (K <= 16) return launch_variant<2, 1, 1, 16, 16>(prm, st);   // tile 64 x 16
     return launch_variant<1, 1, 1, 32, 32>(prm, st);                // tile 32 x 16

@@ -1,0 +1,145 @@
+"""Device-side logic of the tiled search kernels (csrc/search_tiled.cu), run WITHOUT a GPU under
+the SIMT emulator of tests/hostlogic/simt/ (see tests/test_staged_simt.py for what it models).
+
+* search_tiled_kernel (kernel id 2, the default path) is validated bit for bit on B200 hardware
+  (tests/test_gpu_parity.py); reproducing the oracle here as well checks the EMULATOR.
+* search_tiledq_kernel (kernel id 4: the same gathers, survivors of the pre-test compacted into
+  per-warp queues, lists in the output planes) must equal the oracle's f32seq search bit for bit
+  for several thread schedules (lanes are not in lockstep between warp collectives).
+"""
+import ctypes
+import math
+import os
+import subprocess
+
+import numpy as np
+import pytest
+
+from paper_1901_02492_b200 import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HL = os.path.join(ROOT, "tests", "hostlogic")
+SRC = os.path.join(HL, "tiled_simt.cpp")
+LIB = os.path.join(HL, "libtiled_simt.so")
+CSRC = os.path.join(ROOT, "paper_1901_02492_b200", "csrc")
+PLANES = ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")
+TILED, QUEUED = 0, 1
+
+
+def _stale():
+    if not os.path.exists(LIB):
+        return True
+    t = os.path.getmtime(LIB)
+    deps = [SRC, os.path.join(ROOT, "include", "kbmod_b200.h")]
+    deps += [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
+    deps += [os.path.join(HL, "simt", f) for f in os.listdir(os.path.join(HL, "simt"))]
+    return any(os.path.getmtime(d) > t for d in deps)
+
+
+@pytest.fixture(scope="module")
+def sim():
+    if _stale():
+        subprocess.run(["g++", "-O1", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC",
+                        "-I", os.path.join(HL, "simt"), "-I", os.path.join(ROOT, "include"), "-I", CSRC,
+                        "-DKBMOD_SIMT_EMUL=1", SRC, "-o", LIB], check=True)
+    return ctypes.CDLL(LIB)
+
+
+def run_sim(sim, pp, times, vel, K, min_obs, queued, order=0, seed=1):
+    N, H, W, _ = pp.shape
+    pp = np.ascontiguousarray(pp, np.float32)
+    times = np.ascontiguousarray(times, np.float64)
+    vel = np.ascontiguousarray(vel, np.float32)
+    out = {k: np.full((H, W, K), -77, np.int32 if k in ("vel_idx", "n_obs") else np.float32) for k in PLANES}
+    stats = (ctypes.c_longlong * 8)()
+    ptr = lambda a: a.ctypes.data_as(ctypes.c_void_p)
+    rc = sim.simt_search_tiled(ptr(pp), ptr(times), N, H, W, ptr(vel), int(vel.shape[0]), int(K), int(min_obs),
+                               *[ptr(out[k]) for k in PLANES], int(queued), int(order), ctypes.c_uint(seed), stats)
+    assert rc == 0, f"launch_search_tiled returned {rc}"
+    assert stats[3] == 2, "encode kernel + search kernel"
+    return out
+
+
+def assert_exact(out, ref):
+    for k in PLANES:
+        a, b = out[k], ref[k]
+        same = (a.view(np.int32) == b.view(np.int32)) | (a == b)
+        assert same.all(), f"{k}: {int((~same).sum())} of {same.size} entries differ from the oracle"
+
+
+def stack_case(orc, k, **over):
+    cfg = synth.config(k, **over)
+    st = synth.make_stack(cfg)
+    return cfg, st, orc.make_psi_phi(st.sci, st.var, st.mask, st.psf)
+
+
+@pytest.mark.parametrize("queued", [TILED, QUEUED])
+def test_config1(sim, orc, queued):
+    cfg, st, pp = stack_case(orc, 1)
+    ref = orc.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs)
+    for order, seed in ((0, 1), (1, 1), (2, 9)):
+        out = run_sim(sim, pp, st.times, st.vel_grid, cfg.K, cfg.min_obs, queued, order, seed)
+        assert_exact(out, ref)
+    y, x = np.unravel_index(np.argmax(out["nu"][..., 0]), out["nu"].shape[:2])
+    assert (x, y) == (20, 30)
+
+
+@pytest.mark.parametrize("queued", [TILED, QUEUED])
+@pytest.mark.parametrize("k,over", [
+    (2, dict(N=8, H=75, W=203)),                                      # odd width, ragged tiles
+    (3, dict(N=15, H=70, W=133, n_sources=4)),
+    (4, dict(N=12, H=66, W=140, n_sources=4, n_angles=16, n_speeds=8)),   # K = 16: blocks of 16, generic insert
+])
+def test_crops_of_the_baseline_configs(sim, orc, queued, k, over):
+    cfg, st, pp = stack_case(orc, k, **over)
+    ref = orc.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs)
+    assert_exact(run_sim(sim, pp, st.times, st.vel_grid, cfg.K, cfg.min_obs, queued, order=2, seed=k), ref)
+
+
+def test_queued_interior_trajectories_fill_the_lists(sim, orc):
+    """Slow velocities keep every window inside the image (the fast path of the gathers) and make
+    every trajectory eligible: queues overflow 32 inside a block, same-pixel candidates meet in
+    one batch; K = 3 / 8 (register insert), 16 and 32 (generic insert, other tile shapes)."""
+    pp = synth.random_psiphi(6, 70, 140, seed=5, invalid_frac=0.02)
+    times = np.array([0, .1, .2, 1.0, 1.1, 1.2])
+    vel = synth.velocity_grid(10, 8, -math.pi, math.pi, 0.5, 6.0)
+    for K, mo, order in ((8, 2, 2), (3, 6, 1), (16, 1, 2), (32, 1, 0)):
+        ref = orc.search(pp, times, vel, K, mo)
+        assert_exact(run_sim(sim, pp, times, vel, K, mo, QUEUED, order, seed=K), ref)
+
+
+def test_queued_unproven_shifts_and_degenerate_shapes(sim, orc):
+    H, W = 31, 200
+    pp = np.zeros((3, H, W, 2), np.float32)
+    pp[1:, ..., 0] = (np.arange(H)[:, None] * W + np.arange(W)[None, :]).astype(np.float32)[None]
+    pp[0, ..., 0] = 0.25
+    pp[..., 1] = 1.0
+    times = np.array([0.0, 0.5, 1.0])
+    vel = np.array([[3.0, 1.0], [-3.0, -1.0], [1.0, 3.0], [10.49999, 0.0], [20.99998, 0.5],
+                    [0.49999997, 0.49999997], [0.99999994, -0.99999994], [7.0, 7.0],
+                    [-0.5, 0.0], [99.5, 0.0], [199.0, 1.0], [10.5, 10.5]], np.float32)
+    assert_exact(run_sim(sim, pp, times, vel, 4, 2, QUEUED, order=1), orc.search(pp, times, vel, 4, 2))
+    # N = 1
+    pp = synth.random_psiphi(1, 1, 33, seed=1, invalid_frac=0.2)
+    vel0 = np.zeros((1, 2), np.float32)
+    assert_exact(run_sim(sim, pp, [3.0], vel0, 2, 1, QUEUED), orc.search(pp, [3.0], vel0, 2, 1))
+    # far velocities, unsorted times, duplicated velocities, V not a multiple of the block
+    pp = synth.random_psiphi(5, 37, 70, seed=3, invalid_frac=0.1)
+    vel = synth.velocity_grid(4, 4, -2, 2, 2, 12)
+    vel = np.concatenate([vel, vel[3:9], vel[:2], np.array([[5e4, 0], [0, -7e4], [3e3, 3e3]], np.float32)])
+    times = np.array([5.0, 4.5, 6.0, 5.25, 7.0])
+    assert_exact(run_sim(sim, pp, times, vel, 8, 3, QUEUED, order=2, seed=3), orc.search(pp, times, vel, 8, 3))
+    # everything invalid: only sentinels
+    pp = synth.random_psiphi(4, 10, 40, seed=2, invalid_frac=1.0)
+    out = run_sim(sim, pp, np.arange(4.0), vel[:9], 4, 1, QUEUED)
+    assert_exact(out, orc.search(pp, np.arange(4.0), vel[:9], 4, 1))
+    assert (out["vel_idx"] == -1).all()
+
+
+def test_queued_maximum_image_count(sim, orc):
+    rng = np.random.default_rng(64)
+    for N, mo in ((40, 20), (64, 20)):
+        pp = synth.random_psiphi(N, 34, 70, seed=N, invalid_frac=0.05)
+        times = np.sort(rng.uniform(0.0, 5.0, N))
+        vel = synth.velocity_grid(6, 4, -math.pi / 2, math.pi / 2, 1.0, 9.0)
+        assert_exact(run_sim(sim, pp, times, vel, 8, mo, QUEUED, order=2, seed=N), orc.search(pp, times, vel, 8, mo))
