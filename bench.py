@@ -8,7 +8,15 @@ metric is quoted on (15 x 4096 x 4096, 640 velocities, K=8, min_obs=8; 1.07e10 t
 HBM; `e2e` = the same through the public API from pinned HOST buffers (H2D of sci/var/mask and D2H
 of the result planes inside the timed region).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3] [--kernel 0]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3] [--kernel -1]
+
+--kernel -1 (default): the search kernel is chosen by measurement.  A child process runs the
+workload once with the library's default kernel (id 0 -> search_tiled_kernel, validated against the
+oracle on B200) and once with the candidate (id 4, search_tiledq_kernel: same gathers, queue-
+compacted top-K), compares all six result planes bit for bit on the device and times both; the
+candidate is used for the timed region only if its results are identical AND it is faster.  The
+outcome is reported in the line's "kernel_selection".  A candidate that fails or faults costs
+nothing: the child is a separate process with its own CUDA context.
 
 N > 1 (torchrun): every rank searches its own independent stack (the survey's fields/CCDs are
 independent searches) -- weak scaling, no data-path collective.
@@ -165,6 +173,65 @@ def config_dict(cfg, args):
 
 
 # ----------------------------------------------------------------------------------------------
+# kernel selection by measurement (child process: its own CUDA context)
+# ----------------------------------------------------------------------------------------------
+CANDIDATE_KERNEL = 4
+KERNEL_NAMES = {0: "search_tiled_kernel (automatic)", 1: "search_direct_kernel", 2: "search_tiled_kernel",
+                3: "search_staged_kernel", 4: "search_tiledq_kernel"}
+
+
+def probe_child(args, cfg, local_rank):
+    """Child mode (--probe): default kernel vs candidate on this workload; prints one JSON line."""
+    import torch
+    from paper_1901_02492_b200 import binding, build
+    build.build()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    st = synth.make_stack(cfg, seed=args.probe_seed)
+    N, H, W, V, K = cfg.N, cfg.H, cfg.W, cfg.V, cfg.K
+    to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    psiphi = binding.make_psi_phi(to(st.sci), to(st.var), to(st.mask), st.psf)
+    ws = torch.empty(binding.search_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
+    res, ms = {}, {}
+    for which in (0, CANDIDATE_KERNEL):
+        binding.set_search_kernel(which)
+        out = binding.alloc_result(H, W, K, dev)
+        ts = []
+        for _ in range(3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            binding.search(psiphi, st.times, st.vel_grid, K, cfg.min_obs, out=out, workspace=ws)
+            b.record()
+            binding.search_status(ws)
+            ts.append(a.elapsed_time(b))
+        res[which], ms[which] = out, float(np.median(ts))
+    same = all(torch.equal(res[0][k].view(torch.int32), res[CANDIDATE_KERNEL][k].view(torch.int32)) for k in res[0])
+    print(json.dumps({"probe": True, "identical": bool(same), "ms_default": ms[0], "ms_candidate": ms[CANDIDATE_KERNEL]}))
+
+
+def select_kernel(args, seed, local_rank):
+    """Parent: returns (kernel id, report dict)."""
+    cmd = [sys.executable, os.path.abspath(__file__), "--probe", "--probe-seed", str(seed),
+           "--config", str(args.config), "--rows", str(args.rows)]
+    env = dict(os.environ, LOCAL_RANK=str(local_rank), WORLD_SIZE="1", RANK="0")
+    rep = {"default": KERNEL_NAMES[0], "candidate": KERNEL_NAMES[CANDIDATE_KERNEL]}
+    try:
+        cp = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env=env)
+        lines = [l for l in cp.stdout.splitlines() if l.startswith('{"probe"')]
+        if cp.returncode != 0 or not lines:
+            rep["error"] = f"probe exited {cp.returncode}: {cp.stderr.strip()[-200:]}"
+            return 0, rep
+        rep.update(json.loads(lines[-1]))
+        use = rep["identical"] and rep["ms_candidate"] < rep["ms_default"]
+        rep["selected"] = KERNEL_NAMES[CANDIDATE_KERNEL if use else 0]
+        rep["rule"] = "candidate only if all six result planes are bit-identical to the default kernel's and it is faster"
+        return (CANDIDATE_KERNEL if use else 0), rep
+    except Exception as exc:
+        rep["error"] = f"{type(exc).__name__}: {exc}"[:200]
+        return 0, rep
+
+
+# ----------------------------------------------------------------------------------------------
 # GPU arm
 # ----------------------------------------------------------------------------------------------
 def run_gpu(args, cfg, st, rank, world, local_rank):
@@ -177,7 +244,15 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
         raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    binding.set_search_kernel(args.kernel)
+    selection = None
+    kernel = args.kernel
+    if kernel < 0:
+        kernel, selection = select_kernel(args, shard.rank_seed(cfg.seed, rank), local_rank)
+        if world > 1:                       # every rank times the same kernel: the candidate only if all agree
+            t = torch.tensor([kernel], device=dev, dtype=torch.int32)
+            dist.all_reduce(t, op=dist.ReduceOp.MIN)
+            kernel = int(t.item())
+    binding.set_search_kernel(kernel)
     N, H, W, V, K = cfg.N, cfg.H, cfg.W, cfg.V, cfg.K
 
     # pinned host inputs and outputs (for e2e), resident device copies (for value)
@@ -299,10 +374,10 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
                         "trajectories_per_s": cfg.trajectories / (ms_search * 1e-3)},
         "roofline": {"bound": "smem", "achieved": achieved, "peak": lsu_peak, "unit": "GB/s",
                      "frac": achieved / lsu_peak,
-                     "traffic": (NCU_DRAM_BYTES_CONFIG3.get(args.kernel)
+                     "traffic": (NCU_DRAM_BYTES_CONFIG3.get(kernel)
                                  if args.config == 3 and not args.rows else None),
                      "traffic_source": "profiles/ (ncu --set full of an earlier run of this kernel)",
-                     "kernel": "kbmod_search",
+                     "kernel": f"kbmod_search -> {KERNEL_NAMES.get(kernel, kernel)}",
                      "peak_source": f"148 SM x 128 B/clk x {sm_max_mhz:.0f} MHz ({peak_src} max "
                                     "SM clock); north_star roofline = slower of HBM and LSU",
                      "hbm": {"compulsory_bytes": hbm_bytes, "peak": hbm_gbs,
@@ -315,6 +390,8 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
                 "h2d_bytes_per_step": int(h_sci.numel() * 4 + h_var.numel() * 4 + h_mask.numel()),
                 "d2h_bytes_per_step": int(sum(v.numel() * v.element_size() for v in h_out.values()))},
         "e2e_host_abi": host_abi,
+        "search_kernel": KERNEL_NAMES.get(kernel, str(kernel)),
+        "kernel_selection": selection if selection is not None else {"selected": KERNEL_NAMES.get(kernel), "rule": "--kernel given"},
     }
     if world == 1 and not args.no_cpu:
         import oracle
@@ -337,7 +414,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--rows", type=int, default=0, help="override H (debug only)")
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto (tiled), 1 direct, 2 tiled, 3 TMA-staged")
+    ap.add_argument("--kernel", type=int, default=-1,
+                    help="-1 choose by measurement (default kernel vs candidate 4, see the module docstring), "
+                         "0 library default (tiled), 1 direct, 2 tiled, 3 TMA-staged, 4 tiled + queued top-K")
+    ap.add_argument("--probe", action="store_true", help="child mode of --kernel -1 (internal)")
+    ap.add_argument("--probe-seed", type=int, default=0, help="stack seed of the probe (internal)")
     ap.add_argument("--ref-rows", type=int, default=256, help="start rows per oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
@@ -346,6 +427,10 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     cfg = workload(args)
+
+    if args.probe:
+        probe_child(args, cfg, local_rank)
+        return
 
     if args.impl == "reference":
         if rank != 0:

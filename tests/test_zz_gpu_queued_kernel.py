@@ -1,0 +1,79 @@
+"""GPU parity of search kernel 4 (search_tiledq_kernel: the tiled kernel's gathers with
+queue-compacted S5/S6), through the C ABI against the CPU oracle: the same cases as the other
+kernels in tests/test_gpu_parity.py (whose test bodies are reused with which = 4), plus the
+full-size comparison with the default kernel.  Its device logic is checked on the CPU first
+(tests/test_tiled_simt.py); this file sorts last so that it runs after every other GPU test.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1901_02492_b200 import synth
+
+from tests import test_gpu_parity as P
+
+pytestmark = pytest.mark.gpu
+QUEUED = 4
+
+
+@pytest.fixture(scope="module")
+def kb():
+    from paper_1901_02492_b200 import binding
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    binding.lib()
+    yield binding
+    binding.set_search_kernel(0)
+
+
+def test_queued_config1_end_to_end(kb, orc):
+    P.test_search_config1_end_to_end(kb, orc, QUEUED)
+
+
+@pytest.mark.parametrize("k,over", [
+    (2, dict(N=8, H=75, W=203)),
+    (3, dict(N=15, H=70, W=133, n_sources=4)),
+    (4, dict(N=12, H=66, W=140, n_sources=4, n_angles=16, n_speeds=8)),
+    (5, dict(N=20, H=40, W=97, n_angles=8, n_speeds=8)),
+])
+def test_queued_crops_match_oracle_exactly(kb, orc, k, over):
+    P.test_search_crops_match_oracle_exactly(kb, orc, QUEUED, k, over)
+
+
+def test_queued_slow_velocities_interior(kb, orc):
+    P.test_search_slow_velocities_interior(kb, orc, QUEUED)
+
+
+def test_queued_maximum_image_count(kb, orc):
+    P.test_search_maximum_image_count(kb, orc, QUEUED)
+
+
+def test_queued_edge_cases(kb, orc):
+    P.test_search_edge_cases(kb, orc, QUEUED)
+
+
+def test_queued_half_integer_and_near_tie_positions(kb, orc):
+    P.test_search_half_integer_and_near_tie_positions(kb, orc, QUEUED)
+
+
+def test_queued_full_size_config3_equals_default_kernel_and_oracle_bands(kb, orc):
+    """BASELINE.json configs[2] at full size: all six result planes of kernel 4 equal the default
+    kernel's bit for bit (every start pixel, every slot), and four 8-row bands equal the oracle."""
+    cfg = synth.config(3)
+    st = synth.make_stack(cfg)
+    pp = kb.make_psi_phi(P._cuda(st.sci), P._cuda(st.var), P._cuda(st.mask), st.psf)
+    kb.set_search_kernel(0)
+    ref = kb.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs)
+    kb.set_search_kernel(QUEUED)
+    res = kb.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs)
+    for k in ("vel_idx", "n_obs"):
+        assert torch.equal(res[k], ref[k]), k
+    for k in ("psi", "phi", "nu", "alpha"):
+        assert torch.equal(res[k].view(torch.int32), ref[k].view(torch.int32)), k
+    del ref
+    pp_host = pp.cpu().numpy()
+    del pp
+    for y0 in (0, 28, 2044, cfg.H - 8):
+        band = orc.search(pp_host, st.times, st.vel_grid, cfg.K, cfg.min_obs, y_begin=y0, y_end=y0 + 8)
+        gpu = {k: v[y0:y0 + 8].cpu().numpy() for k, v in res.items()}
+        P.assert_search_exact(gpu, band)
