@@ -489,12 +489,18 @@ __device__ __forceinline__ void process_batch_q(const TiledParams& prm, const fl
     }
 }
 
-// RX x RY pixels per thread: x = tile_x + rx * 32 + lane, y = tile_y + warp * RY + ry; B * RX * RY = 32
-template <int RX, int RY, int B, int KP>
+// RX x RY pixels per thread: x = tile_x + rx * 32 + lane, y = tile_y + warp * RY + ry; B * RX * RY = 32.
+// CM: how valid samples are counted.  0: one additive counter per (velocity, pixel).  2 (RX = 2,
+// N <= 16): the sign bits are shifted into a history word shared by the two rx pixels of a row
+// (rx = 0 lands on the odd bits, rx = 1 on the even ones) and counted with popc when the block is
+// scored: half the counter registers, so more gathers can be in flight.
+template <int RX, int RY, int B, int KP, int CM>
 __global__ void __launch_bounds__(THREADS, 1)
 search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
     constexpr int R = RX * RY;
     static_assert(B * R == 32, "the scoring switch lists B*R = 32 steps");
+    static_assert(CM == 0 || (CM == 2 && RX == 2), "history counting pairs the two rx pixels of a row");
+    constexpr int NC = (CM == 2) ? RY : R;        // count registers per velocity
     constexpr int TW = 32 * RX, TH = RY * (THREADS / 32);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = prm.N, H = prm.H, W = prm.W, K = prm.K;
@@ -565,8 +571,14 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
         }
 
         u64 acc[B][R];
-        unsigned cnt[B][R];
+        unsigned cnt[B][NC];
         unsigned fast = 0;          // bit b: every window of velocity b is inside the image
+        // one sample of pixel r (= ry * RX + rx) of velocity b: the packed add and the validity count
+        auto take = [&](int b, int r, u64 s) {
+            acc_add(acc[b][r], s);
+            if constexpr (CM == 2) cnt[b][r / RX] = __funnelshift_l((unsigned)(s >> 32), cnt[b][r / RX], 1);
+            else cnt[b][r] += (unsigned)(s >> 63);
+        };
 #pragma unroll
         for (int b = 0; b < B; ++b) {
 #pragma unroll
@@ -574,7 +586,8 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
                 // image 0 has dt = 0: shift (0,0) for every velocity
                 const u64 s0 = (inimg & (1u << r)) ? ld_sample(basep[r / RX] + 32 * (r % RX)) : 0ull;
                 acc[b][r] = s0;
-                cnt[b][r] = (unsigned)(s0 >> 63);
+                if constexpr (CM == 2) cnt[b][r / RX] = (r % RX) ? cnt[b][r / RX] * 2u + (unsigned)(s0 >> 63) : (unsigned)(s0 >> 63);
+                else cnt[b][r] = (unsigned)(s0 >> 63);
             }
             const int bx = r_meta[b * META + 1], by = r_meta[b * META + 2];
             const int sxlo = (short)(bx & 0xFFFF), sxhi = bx >> 16;
@@ -584,6 +597,26 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
             fast |= ok ? (1u << b) : 0u;
         }
 
+        if (fast == (B == 32 ? 0xFFFFFFFFu : (1u << B) - 1u)) {
+            // every window of every velocity of the block is inside the image (interior tiles):
+            // straight-line code per image, so the B x R independent loads can be issued ahead of
+            // the adds (the per-velocity branches of the general loop below keep only R in flight)
+            for (int i = 1; i < N; ++i) {
+#pragma unroll
+                for (int b = 0; b < B; ++b) {
+                    const int o = r_off[b * N + i];
+#pragma unroll
+                    for (int ry = 0; ry < RY; ++ry) {
+                        const u64* p = basep[ry] + o;
+#pragma unroll
+                        for (int rx = 0; rx < RX; ++rx) {
+                            const u64 s = ld_sample(p + 32 * rx);
+                            take(b, ry * RX + rx, s);
+                        }
+                    }
+                }
+            }
+        } else
         for (int i = 1; i < N; ++i) {
 #pragma unroll
             for (int b = 0; b < B; ++b) {
@@ -595,8 +628,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
 #pragma unroll
                         for (int rx = 0; rx < RX; ++rx) {
                             const u64 s = ld_sample(p + 32 * rx);
-                            acc_add(acc[b][ry * RX + rx], s);
-                            cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
+                            take(b, ry * RX + rx, s);
                         }
                     }
                 } else {
@@ -617,8 +649,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
                                 const int x = x_first + 32 * rx + sx;
                                 const bool in = yin && (x_first + 32 * rx < W) && x >= 0 && x < W;
                                 const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
-                                acc_add(acc[b][ry * RX + rx], s);
-                                cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
+                                take(b, ry * RX + rx, s);
                             }
                         }
                     } else {
@@ -635,8 +666,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
                                 const bool in = traj_pixel(x_first + 32 * rx, vx, dti, W, x) && yin &&
                                                 (x_first + 32 * rx < W);
                                 const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
-                                acc_add(acc[b][ry * RX + rx], s);
-                                cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
+                                take(b, ry * RX + rx, s);
                             }
                         }
                     }
@@ -659,7 +689,10 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
         if (j >= 0) {                                                                                    \
             const float Psi = __uint_as_float((unsigned)acc[b_][r_]);                                    \
             const float Phi = 0.0f - __uint_as_float((unsigned)(acc[b_][r_] >> 32));                     \
-            const bool pass = (cnt[b_][r_] >= minobs) && (Phi > 0.0f) && ((inimg >> r_) & 1u) &&         \
+            unsigned n;                                                                                  \
+            if constexpr (CM == 2) n = __popc(cnt[b_][r_ / RX] & ((r_ % RX) ? 0x55555555u : 0xAAAAAAAAu)); \
+            else n = cnt[b_][r_ % NC];                                                                   \
+            const bool pass = (n >= minobs) && (Phi > 0.0f) && ((inimg >> r_) & 1u) &&                   \
                               !(Psi * rsqrtf(Phi) < lo[r_]);                                             \
             const unsigned m = __ballot_sync(0xFFFFFFFFu, pass);                                         \
             if (m) {                                                                                     \
@@ -766,12 +799,12 @@ static int launch_variant(TiledParams& prm, cudaStream_t st) {
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }
 
-template <int RX, int RY, int B, int KP>
+template <int RX, int RY, int B, int KP, int CM>
 static int launch_variant_q(TiledParams& prm, cudaStream_t st) {
     constexpr int TW = 32 * RX, TH = RY * (THREADS / 32);
     const size_t smem = rec_ints(B, prm.N) * sizeof(int) + (size_t)(THREADS / 32) * QCAP * 12;
     if (smem > 227 * 1024) return KBMOD_ERR_UNSUPPORTED;
-    auto kern = search_tiledq_kernel<RX, RY, B, KP>;
+    auto kern = search_tiledq_kernel<RX, RY, B, KP, CM>;
     static bool attr_set = false;
     if (!attr_set) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess)
@@ -816,9 +849,10 @@ int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, i
     prm.out = out;
     prm.dt = dt;
     if (queued) {                                                   // kernel 4: same tiles, queue-compacted S5/S6
-        if (K <= 8) return launch_variant_q<2, 2, 8, 8>(prm, st);
-        if (K <= 16) return launch_variant_q<2, 1, 16, 0>(prm, st);
-        return launch_variant_q<1, 1, 32, 0>(prm, st);
+        const bool hist = N <= 16;                                  // history-bit counting (see CM)
+        if (K <= 8) return hist ? launch_variant_q<2, 2, 8, 8, 2>(prm, st) : launch_variant_q<2, 2, 8, 8, 0>(prm, st);
+        if (K <= 16) return hist ? launch_variant_q<2, 1, 16, 0, 2>(prm, st) : launch_variant_q<2, 1, 16, 0, 0>(prm, st);
+        return launch_variant_q<1, 1, 32, 0, 0>(prm, st);
     }
     if (K <= 8) return launch_variant<2, 2, 1, 8, 8>(prm, st);      // tile 64 x 32
     if (K <= 16) return launch_variant<2, 1, 1, 16, 16>(prm, st);   // tile 64 x 16

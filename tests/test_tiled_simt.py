@@ -100,7 +100,7 @@ def test_queued_interior_trajectories_fill_the_lists(sim, orc):
     """Slow velocities keep every window inside the image (the fast path of the gathers) and make
     every trajectory eligible: queues overflow 32 inside a block, same-pixel candidates meet in
     one batch; K = 3 / 8 (register insert), 16 and 32 (generic insert, other tile shapes)."""
-    pp = synth.random_psiphi(6, 70, 140, seed=5, invalid_frac=0.02)
+    pp = synth.random_psiphi(6, 100, 140, seed=5, invalid_frac=0.02)    # tiles (1,1), (1,2): all windows inside
     times = np.array([0, .1, .2, 1.0, 1.1, 1.2])
     vel = synth.velocity_grid(10, 8, -math.pi, math.pi, 0.5, 6.0)
     for K, mo, order in ((8, 2, 2), (3, 6, 1), (16, 1, 2), (32, 1, 0)):
@@ -136,10 +136,13 @@ def test_queued_unproven_shifts_and_degenerate_shapes(sim, orc):
     assert (out["vel_idx"] == -1).all()
 
 
-def test_queued_maximum_image_count(sim, orc):
+def test_queued_image_count_variants(sim, orc):
+    """N = 16 (the largest stack counted with history bits), 17 and above (additive counters),
+    N = 64 = KBMOD_MAX_IMAGES; slow velocities and a 100 x 140 image so interior tiles take the
+    branch-free path in both counting modes."""
     rng = np.random.default_rng(64)
-    for N, mo in ((40, 20), (64, 20)):
-        pp = synth.random_psiphi(N, 34, 70, seed=N, invalid_frac=0.05)
+    for N, mo in ((16, 16), (17, 9), (40, 20), (64, 20)):
+        pp = synth.random_psiphi(N, 100 if N < 20 else 34, 140 if N < 20 else 70, seed=N, invalid_frac=0.05)
         times = np.sort(rng.uniform(0.0, 5.0, N))
         vel = synth.velocity_grid(6, 4, -math.pi / 2, math.pi / 2, 1.0, 9.0)
         assert_exact(run_sim(sim, pp, times, vel, 8, mo, QUEUED, order=2, seed=N), orc.search(pp, times, vel, 8, mo))
