@@ -573,6 +573,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
         u64 acc[B][R];
         unsigned cnt[B][NC];
         unsigned fast = 0;          // bit b: every window of velocity b is inside the image
+        bool proven = true;         // every (velocity, image >= 1) of the block has a proven integer shift
         // one sample of pixel r (= ry * RX + rx) of velocity b: the packed add and the validity count
         auto take = [&](int b, int r, u64 s) {
             acc_add(acc[b][r], s);
@@ -595,6 +596,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
             const bool ok = r_meta[b * META + 3] && !ragged && tile_x + sxlo >= 0 &&
                             tile_x1 + sxhi < W && tile_y + sylo >= 0 && tile_y1 + syhi < H;
             fast |= ok ? (1u << b) : 0u;
+            proven = proven && (r_meta[b * META + 3] != 0);
         }
 
         if (fast == (B == 32 ? 0xFFFFFFFFu : (1u << B) - 1u)) {
@@ -611,6 +613,29 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
 #pragma unroll
                         for (int rx = 0; rx < RX; ++rx) {
                             const u64 s = ld_sample(p + 32 * rx);
+                            take(b, ry * RX + rx, s);
+                        }
+                    }
+                }
+            }
+        } else if (proven) {
+            // every shift of the block is proven but some windows cross the image border (or the
+            // tile is ragged): still straight-line code, each lane tests its own sample position
+            for (int i = 1; i < N; ++i) {
+#pragma unroll
+                for (int b = 0; b < B; ++b) {
+                    const int o = r_off[b * N + i];
+                    const int code = r_sh[b * N + i];
+                    const int sx = (short)(code & 0xFFFF), sy = code >> 16;
+#pragma unroll
+                    for (int ry = 0; ry < RY; ++ry) {
+                        const bool yin = (unsigned)(y_first + ry + sy) < (unsigned)H;
+                        const u64* p = basep[ry] + o;       // = enc + ((i*H + y)*W + x) for pixels inside the image
+#pragma unroll
+                        for (int rx = 0; rx < RX; ++rx) {
+                            const bool in = yin && ((inimg >> (ry * RX + rx)) & 1u) &&
+                                            (unsigned)(x_first + 32 * rx + sx) < (unsigned)W;
+                            const u64 s = in ? ld_sample(p + 32 * rx) : 0ull;
                             take(b, ry * RX + rx, s);
                         }
                     }
