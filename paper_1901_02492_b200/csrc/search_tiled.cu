@@ -506,8 +506,8 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
     const int N = prm.N, H = prm.H, W = prm.W, K = prm.K;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int rec_n = (int)rec_ints(B, N);
-    int* rec = reinterpret_cast<int*>(smem_raw);                  // off[B][N], sh[B][N], meta[B][META]
-    float* q_psi = reinterpret_cast<float*>(rec + rec_n) + warp * (3 * QCAP);
+    int* rec2 = reinterpret_cast<int*>(smem_raw);                 // two block records (double buffer)
+    float* q_psi = reinterpret_cast<float*>(rec2 + 2 * rec_n) + warp * (3 * QCAP);
     float* q_phi = q_psi + QCAP;
     unsigned* q_meta = reinterpret_cast<unsigned*>(q_phi + QCAP);
 
@@ -549,17 +549,21 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
     unsigned qhead = 0, qtail = 0;
     const unsigned minobs = (unsigned)prm.min_obs;
 
-    int* r_off = rec;
-    int* r_sh = rec + B * N;
-    int* r_meta = rec + 2 * B * N;
+    // block records are double-buffered: record blk+1 is fetched while block blk is computed, and
+    // one barrier per block both publishes it and retires record blk
+    for (int k = tid; k < rec_n; k += THREADS) rec2[k] = __ldg(prm.plan + k);
+    __syncthreads();
 
     for (int blk = 0; blk < prm.nblk; ++blk) {
-        __syncthreads();
-        {
-            const int* src = prm.plan + (size_t)blk * rec_n;
-            for (int k = tid; k < rec_n; k += THREADS) rec[k] = __ldg(src + k);
+        const int* rec = rec2 + (blk & 1) * rec_n;                // off[B][N], sh[B][N], meta[B][META]
+        const int* r_off = rec;
+        const int* r_sh = rec + B * N;
+        const int* r_meta = rec + 2 * B * N;
+        if (blk + 1 < prm.nblk) {
+            const int* src = prm.plan + (size_t)(blk + 1) * rec_n;
+            int* dst = rec2 + ((blk + 1) & 1) * rec_n;
+            for (int k = tid; k < rec_n; k += THREADS) dst[k] = __ldg(src + k);
         }
-        __syncthreads();
 
         float lo[R];                               // pre-test bound: K-th best nu minus a safety margin
 #pragma unroll
@@ -752,7 +756,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
             process_batch_q<RX, KP>(prm, q_psi, q_phi, q_meta, qhead, 32, lane, tile_x, y_first);
             qhead += 32;
         }
-        __syncwarp();
+        __syncthreads();
     }
 
     // ---- end of tile: drain the queue, then re-evaluate the winners literally and write them
@@ -827,15 +831,11 @@ static int launch_variant(TiledParams& prm, cudaStream_t st) {
 template <int RX, int RY, int B, int KP, int CM>
 static int launch_variant_q(TiledParams& prm, cudaStream_t st) {
     constexpr int TW = 32 * RX, TH = RY * (THREADS / 32);
-    const size_t smem = rec_ints(B, prm.N) * sizeof(int) + (size_t)(THREADS / 32) * QCAP * 12;
-    if (smem > 227 * 1024) return KBMOD_ERR_UNSUPPORTED;
+    // two block records + the queues: 14.7 KB at N = 15, 46.8 KB at most (N = 64, B = 32), i.e. below
+    // the 48 KB that need no opt-in; the rest of the SM's 256 KB stays L1 for the gathers
+    const size_t smem = 2 * rec_ints(B, prm.N) * sizeof(int) + (size_t)(THREADS / 32) * QCAP * 12;
+    if (smem > 48 * 1024) return KBMOD_ERR_UNSUPPORTED;
     auto kern = search_tiledq_kernel<RX, RY, B, KP, CM>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess)
-            return KBMOD_ERR_CUDA;
-        attr_set = true;
-    }
     prm.tiles_x = (prm.W + TW - 1) / TW;
     prm.tiles_y = (prm.H + TH - 1) / TH;
     prm.group_w = std::max(1, 512 / TW);
