@@ -535,6 +535,13 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
     for (int ry = 0; ry < RY; ++ry)
         basep[ry] = prm.enc + (size_t)min(y_first + ry, H - 1) * W + min(x_first, W - 1);
 
+#if !defined(KBMOD_SIMT_EMUL)
+    // keep the row pointers as opaque 64-bit registers: `basep[ry] + o` is then one IMAD.WIDE per
+    // pair of gathers instead of a 64-bit index add plus a 64-bit scale-and-add (4 instructions)
+#pragma unroll
+    for (int ry = 0; ry < RY; ++ry) asm volatile("" : "+l"(basep[ry]));
+#endif
+
     // empty lists (in the output planes)
 #pragma unroll
     for (int r = 0; r < R; ++r)
