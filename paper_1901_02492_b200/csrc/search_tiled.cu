@@ -24,6 +24,7 @@
 //     common path.  Psi/Phi/n_obs of the K winners are re-evaluated once at the end.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -845,7 +846,14 @@ static int launch_variant_q(TiledParams& prm, cudaStream_t st) {
     auto kern = search_tiledq_kernel<RX, RY, B, KP, CM>;
     prm.tiles_x = (prm.W + TW - 1) / TW;
     prm.tiles_y = (prm.H + TH - 1) / TH;
+    // tile rasterisation: groups of group_w tile columns (default 512 px wide).  KBMOD_TILED_GROUPW
+    // (1..256, kernel 4 only) overrides it: a tuning knob bench.py's kernel selection sweeps; the
+    // results do not depend on it
     prm.group_w = std::max(1, 512 / TW);
+    if (const char* e = std::getenv("KBMOD_TILED_GROUPW")) {
+        const int g = std::atoi(e);
+        if (g >= 1 && g <= 256) prm.group_w = g;
+    }
     const long long tiles = (long long)prm.tiles_x * prm.tiles_y;
     if (tiles > 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
     KBMOD_LAUNCH(kern, (unsigned)tiles, THREADS, smem, st, prm);

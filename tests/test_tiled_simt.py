@@ -177,3 +177,12 @@ def test_queued_randomized_shapes(sim, orc):
         pp, times, vel, K, mo = random_case(rng)
         out = run_sim(sim, pp, times, vel, K, mo, QUEUED, int(rng.integers(3)), int(rng.integers(1 << 30)))
         assert_exact(out, orc.search(pp, times, vel, K, mo))
+
+
+@pytest.mark.parametrize("gw", ["1", "3", "200"])
+def test_queued_tile_order_knob_does_not_change_results(sim, orc, gw, monkeypatch):
+    """KBMOD_TILED_GROUPW only permutes which CTA takes which tile (bench.py sweeps it for speed)."""
+    monkeypatch.setenv("KBMOD_TILED_GROUPW", gw)
+    cfg, st, pp = stack_case(orc, 3, N=15, H=70, W=300, n_sources=4)        # 5 x 3 tiles, ragged on both axes
+    ref = orc.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs)
+    assert_exact(run_sim(sim, pp, st.times, st.vel_grid, cfg.K, cfg.min_obs, QUEUED, order=2, seed=int(gw)), ref)
