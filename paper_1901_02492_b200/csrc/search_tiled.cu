@@ -69,13 +69,18 @@ unsigned hilbert_d(unsigned x, unsigned y) {
 
 size_t tiled_plan_bytes(int N, int V, int K) {
     const int B = block_size_for_k(K);
-    const size_t nblk = ((size_t)V + B - 1) / B;
+    const size_t nblk = 2 * (((size_t)V + B - 1) / B);   // kernel 4 may split a block in two (see build_plan)
     return nblk * rec_ints(B, N) * sizeof(int) + 256;
 }
 
 // Builds the host plan; returns the number of velocity blocks.  margin: see the header comment.
+// isolate (kernel 4): a chunk of B velocities that contains velocities with an unproven or skipped
+// shift is split into a block of the clean ones and a block of the others, and blocks are filled
+// up with "benign" padding (never scored, proven shift (0,0): it samples the thread's own pixel),
+// so that the clean block keeps the branch-free gather loops.  The per-pixel result does not
+// depend on the order in which velocities are visited.
 static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, int B,
-                      std::vector<int>& plan) {
+                      std::vector<int>& plan, bool isolate = false) {
     // processing order: Hilbert curve over the velocity plane (ties and order of equal keys: index)
     float lox = vel[0], hix = vel[0], loy = vel[1], hiy = vel[1];
     for (int j = 1; j < V; ++j) {
@@ -96,21 +101,60 @@ static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, 
     const double ulp = std::ldexp(1.0, (int)std::floor(std::log2(cmax)) - 23);
     const double margin = 4.0 * ulp;   // the two roundings move the sum by at most 1 ulp(cmax)
 
-    const int nblk = (V + B - 1) / B;
+    // members of every block: a velocity index, PAD_SKIP (never scored, never sampled) or PAD_BENIGN
+    constexpr int PAD_SKIP = -1, PAD_BENIGN = -2;
+    std::vector<int> members;
+    {
+        auto dirty = [&](int j) {                // some image >= 1 has no proven in-range shift
+            for (int i = 1; i < N; ++i) {
+                volatile float dxf = vel[2 * j] * dt.dt[i];
+                volatile float dyf = vel[2 * j + 1] * dt.dt[i];
+                const double dx = dxf, dy = dyf;
+                if (!(std::fabs(dx) < SH_LIMIT && std::fabs(dy) < SH_LIMIT)) return true;
+                const double fx = dx - std::floor(dx), fy = dy - std::floor(dy);
+                if (std::fabs(fx - 0.5) <= margin || std::fabs(fy - 0.5) <= margin) return true;
+            }
+            return false;
+        };
+        for (int c0 = 0; c0 < V; c0 += B) {
+            const int c1 = std::min(V, c0 + B);
+            std::vector<int> a, d;
+            for (int jj = c0; jj < c1; ++jj) {
+                const int j = key[jj].second;
+                ((isolate && dirty(j)) ? d : a).push_back(j);
+            }
+            if (!a.empty()) {
+                a.resize(B, isolate ? PAD_BENIGN : PAD_SKIP);
+                members.insert(members.end(), a.begin(), a.end());
+            }
+            if (!d.empty()) {
+                d.resize(B, PAD_SKIP);
+                members.insert(members.end(), d.begin(), d.end());
+            }
+        }
+    }
+    const int nblk = (int)(members.size() / B);
     plan.assign((size_t)nblk * rec_ints(B, N), 0);
     for (int blk = 0; blk < nblk; ++blk) {
         int* off = plan.data() + (size_t)blk * rec_ints(B, N);
         int* sh = off + (size_t)B * N;
         int* meta = sh + (size_t)B * N;
         for (int b = 0; b < B; ++b) {
-            const int jj = blk * B + b;
+            const int j = members[(size_t)blk * B + b];
             int* m = meta + b * META;
-            if (jj >= V) {                       // padding velocity: never scored, never sampled
+            if (j == PAD_SKIP) {                 // padding velocity: never scored, never sampled
                 m[0] = -1; m[3] = 0;
                 for (int i = 0; i < N; ++i) { off[b * N + i] = 0; sh[b * N + i] = SH_SKIP; }
                 continue;
             }
-            const int j = key[jj].second;
+            if (j == PAD_BENIGN) {               // never scored; samples the thread's own pixel of image i
+                m[0] = -1; m[1] = 0; m[2] = 0; m[3] = 1;
+                for (int i = 0; i < N; ++i) {
+                    off[b * N + i] = (int)((long long)i * H * W);
+                    sh[b * N + i] = 0;           // proven shift (0, 0)
+                }
+                continue;
+            }
             const float vx = vel[2 * j], vy = vel[2 * j + 1];
             m[0] = j;
             std::memcpy(&m[4], &vx, 4);
@@ -870,7 +914,7 @@ int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, i
     if ((long long)(N + 1) * H * W + (long long)SH_LIMIT * (W + 1) >= 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
     const int B = block_size_for_k(K);
     std::vector<int> plan;
-    const int nblk = build_plan(dt, N, H, W, vel_host, V, B, plan);
+    const int nblk = build_plan(dt, N, H, W, vel_host, V, B, plan, queued);
     if (cudaMemcpyAsync(plan_dev, plan.data(), plan.size() * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
 
