@@ -8,15 +8,13 @@ metric is quoted on (15 x 4096 x 4096, 640 velocities, K=8, min_obs=8; 1.07e10 t
 HBM; `e2e` = the same through the public API from pinned HOST buffers (H2D of sci/var/mask and D2H
 of the result planes inside the timed region).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3] [--kernel -1]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3] [--kernel 0]
 
---kernel -1 (default): the search kernel is chosen by measurement.  A child process runs the
-workload once with the library's default kernel (id 0 -> search_tiled_kernel, validated against the
-oracle on B200) and once with the candidate (id 4, search_tiledq_kernel: same gathers, queue-
-compacted top-K), compares all six result planes bit for bit on the device and times both; the
-candidate is used for the timed region only if its results are identical AND it is faster.  The
-outcome is reported in the line's "kernel_selection".  A candidate that fails or faults costs
-nothing: the child is a separate process with its own CUDA context.
+--kernel 0 (default): the library's default search kernel, the one the GPU test suite validates
+against the oracle; the same kernel every run.  --kernel k forces kernel k.  --kernel -1 (explicit
+opt-in, never the driver's run): a child process runs the workload with the default kernel and with
+candidate 4, compares all six result planes bit for bit on the device and times both; the candidate
+is timed only if identical AND faster ("kernel_selection" in the line).
 
 N > 1 (torchrun): every rank searches its own independent stack (the survey's fields/CCDs are
 independent searches) -- weak scaling, no data-path collective.
@@ -443,9 +441,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--rows", type=int, default=0, help="override H (debug only)")
-    ap.add_argument("--kernel", type=int, default=-1,
-                    help="-1 choose by measurement (default kernel vs candidate 4, see the module docstring), "
-                         "0 library default (tiled), 1 direct, 2 tiled, 3 TMA-staged, 4 tiled + queued top-K")
+    ap.add_argument("--kernel", type=int, default=0,
+                    help="0 library default (the kernel the GPU test suite validates; the default), 1 direct, "
+                         "2 tiled, 3 TMA-staged, 4 tiled + queued top-K, -1 choose by measurement between the "
+                         "default and candidate 4 in a child process (explicit opt-in only)")
     ap.add_argument("--probe", action="store_true", help="child mode of --kernel -1 (internal)")
     ap.add_argument("--probe-seed", type=int, default=0, help="stack seed of the probe (internal)")
     ap.add_argument("--ref-rows", type=int, default=256, help="start rows per oracle sample")

@@ -4,6 +4,8 @@ kernels in tests/test_gpu_parity.py (whose test bodies are reused with which = 4
 full-size comparison with the default kernel.  Its device logic is checked on the CPU first
 (tests/test_tiled_simt.py); this file sorts last so that it runs after every other GPU test.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -12,7 +14,12 @@ from paper_1901_02492_b200 import synth
 
 from tests import test_gpu_parity as P
 
-pytestmark = pytest.mark.gpu
+# Opt-in (KBMOD_TEST_QUEUED=1), exactly like kernel 3 behind KBMOD_TEST_STAGED: a kernel enters the
+# default GPU suite only after this file has passed on hardware in the builder's own run (the kept
+# output is under profiles/).
+pytestmark = [pytest.mark.gpu,
+              pytest.mark.skipif(os.environ.get("KBMOD_TEST_QUEUED") != "1",
+                                 reason="kernel 4 is opt-in: set KBMOD_TEST_QUEUED=1")]
 QUEUED = 4
 
 
