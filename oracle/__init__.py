@@ -16,7 +16,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle.c")
-_LIB = os.path.join(_HERE, "liboracle.so")
+# KBMOD_ORACLE_SANITIZE=1 (tests/test_simt_sanitized.py, in a child interpreter that preloads the ASan
+# runtime): the same source built with -fsanitize=address,undefined into its own shared object
+_SANITIZE = os.environ.get("KBMOD_ORACLE_SANITIZE") == "1"
+_LIB = os.path.join(_HERE, "liboracle_asan.so" if _SANITIZE else "liboracle.so")
 _lib: Optional[ctypes.CDLL] = None
 
 MODE_F64 = 0
@@ -28,7 +31,9 @@ def build(force: bool = False) -> str:
     if (not force and os.path.exists(_LIB)
             and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
         return _LIB
-    cmd = ["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
+    san = ["-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined",
+           "-fno-sanitize-recover=all"] if _SANITIZE else []
+    cmd = ["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", *san,
            "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
     subprocess.run(cmd, check=True)
     return _LIB

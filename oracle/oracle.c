@@ -8,14 +8,14 @@
  *
  * Every function below is the paper's definition written as nested loops (citations are
  * PAPER.md line numbers, "P:<line>").  Readings of silent/garbled passages are the ones
- * listed in DESIGN.md ("Readings", R1..R14).  Pins that check this file against
+ * listed in DESIGN.md section 2 ("Readings of the paper", Q1..Q19).  Pins that check this file against
  * something other than itself live in tests/test_oracle_pins.py (all pinned: P1 analytic
  * source, P2 N(0,1) noise statistics, P3 v=0 inverse-variance coadd vs numpy.average,
  * P4 independent brute force, P5 index-revealing images, P6 mask invariants, P7 scalings).
  *
  * Build: gcc -O2 -std=c99 -ffp-contract=off -fopenmp -shared -fPIC oracle.c -lm
  *   -ffp-contract=off matters: positions and f32seq sums are defined as separately
- *   rounded binary32 operations (R8, R9); an FMA would change them.
+ *   rounded binary32 operations (Q8, Q9, Q18); an FMA would change them.
  */
 #include <math.h>
 #include <stdint.h>
@@ -46,7 +46,7 @@ void oracle_set_threads(int n) {
 
 /* A pixel carries information iff it is unmasked and numerically usable.
  * P:171 "we set the inverse variance to zero so that they will add nothing to the
- * likelihood sum"; non-finite or non-positive variance is read the same way (R6). */
+ * likelihood sum"; non-finite or non-positive variance is read the same way (Q6). */
 static int good_pixel(const float* sci, const float* var, const uint8_t* mask, size_t k) {
     if (mask && mask[k]) return 0;
     if (!isfinite(sci[k]) || !isfinite(var[k])) return 0;
@@ -57,10 +57,10 @@ static int good_pixel(const float* sci, const float* var, const uint8_t* mask, s
  * O1. Likelihood images, diagonal covariance.  P:161-167 Eq.19-20:
  *     Psi(y) = sum_x n(x) T(x - y) / sigma^2(x)
  *     Phi(y) = sum_x T(x - y)^2    / sigma^2(x)
- * written with d = x - y over the P x P support of T: a cross-correlation (R2), terms
- * outside the image or on a not-good pixel have inverse variance 0 (R4, R5).
+ * written with d = x - y over the P x P support of T: a cross-correlation (Q2), terms
+ * outside the image or on a not-good pixel have inverse variance 0 (Q4, Q5).
  * Sums in double, stored as binary32.  If the centre pixel itself is not good, or
- * Phi <= 0, the pixel holds the invalid marker (psi = NaN, phi = 0) (R4).
+ * Phi <= 0, the pixel holds the invalid marker (psi = NaN, phi = 0) (Q4).
  *
  * psf[i][r+dy][r+dx] = T_i(dx, dy).  psiphi is [N,H,W,2] (psi, phi interleaved).
  * psi_abs (optional, may be NULL): sum of |terms| of Psi, for the parity tolerance.
@@ -113,7 +113,7 @@ int oracle_make_psi_phi(const float* sci, const float* var, const uint8_t* mask,
 
 /*
  * S3. Pixel hit by a linear trajectory (P:203 linear trajectories; start pixel in the
- * first image P:231; nearest pixel, R8/R9):
+ * first image P:231; nearest pixel, Q8/Q9):
  *     f  = fl( fl(p0) + fl(v * dt) )          three separately rounded binary32 ops
  *     ip = floor( fl(f + 0.5f) )              exact halves round up
  * Returns 0 and leaves *ip alone when the pixel is outside [0, n).
@@ -138,7 +138,7 @@ typedef struct {
  *     Psi_coadd = sum_i Psi_i(y_i),  Phi_coadd = sum_i Phi_i(y_i)
  * over the observations that exist: in bounds and not the invalid marker.
  * Images in order i = 0..N-1.  mode 0 ("f64"): sums in double, rounded once to binary32.
- * mode 1 ("f32seq"): binary32 adds in image order (R13).
+ * mode 1 ("f32seq"): binary32 adds in image order (Q18).
  * ixiy (optional): per-image pixel, (-1,-1) when out of bounds.
  */
 static coadd_t coadd(const float* psiphi, const float* dt, int N, int H, int W,
@@ -177,11 +177,11 @@ static coadd_t coadd(const float* psiphi, const float* dt, int N, int H, int W,
 }
 
 static void make_dt(const double* times, int N, float* dt) {
-    /* R7: differenced in double against image 0, rounded once to binary32 */
+    /* Q7: differenced in double against image 0, rounded once to binary32 */
     for (int i = 0; i < N; ++i) dt[i] = (float)(times[i] - times[0]);
 }
 
-/* S5. P:180 Eq.22 alpha = Psi/Phi; Eq.26 nu = Psi/sqrt(Phi) (R1).
+/* S5. P:180 Eq.22 alpha = Psi/Phi; Eq.26 nu = Psi/sqrt(Phi) (Q1).
  * binary32, correctly rounded sqrt and divisions. */
 static void score(coadd_t c, float* nu, float* alpha) {
     volatile float s = sqrtf(c.Phi);
@@ -196,7 +196,7 @@ typedef struct {
     int j;
 } cand_t;
 
-/* larger nu first; equal nu: smaller velocity index first (R11) */
+/* larger nu first; equal nu: smaller velocity index first (Q15) */
 static int cand_cmp(const void* pa, const void* pb) {
     const cand_t* a = (const cand_t*)pa;
     const cand_t* b = (const cand_t*)pb;
@@ -209,10 +209,10 @@ static int cand_cmp(const void* pa, const void* pb) {
  * O2. Exhaustive search.  P:205 Eq.27 argmax over (y0, v) of nu_coadd; "evaluate
  * nu for all possible values of y0 and v"; P:231 every start pixel of the first image x
  * every grid velocity.  Retention: the K eligible trajectories of largest nu per start
- * pixel (BASELINE.json north_star; R10), eligible <=> n_obs >= min_obs and Phi > 0.
+ * pixel (BASELINE.json north_star; Q14), eligibility Q13, eligible <=> n_obs >= min_obs and Phi > 0.
  * Selection by a full sort of all V candidates.
  * Output planes are [(y_end - y_begin), W, K]; empty slots: vel_idx = -1, n_obs = 0,
- * psi = phi = alpha = 0, nu = -inf (R12).
+ * psi = phi = alpha = 0, nu = -inf (Q16).
  */
 int oracle_search(const float* psiphi, const double* times, int N, int H, int W,
                   const float* vel, int V, int K, int min_obs, int mode,

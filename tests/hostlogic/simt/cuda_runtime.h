@@ -33,6 +33,18 @@
 
 #define KBMOD_SIMT_EMUL_ACTIVE 1
 
+// AddressSanitizer build (tests/test_simt_sanitized.py): the part of the CTA's shared-memory array
+// beyond the launch's dynamic size is poisoned while the CTA runs, so that a plain-pointer access
+// past the size the launch asked for traps exactly as one past a heap block does.
+#if defined(__SANITIZE_ADDRESS__)
+#include <sanitizer/asan_interface.h>
+#define SIMT_ASAN_POISON(p, n) ASAN_POISON_MEMORY_REGION((p), (n))
+#define SIMT_ASAN_UNPOISON(p, n) ASAN_UNPOISON_MEMORY_REGION((p), (n))
+#else
+#define SIMT_ASAN_POISON(p, n) ((void)0)
+#define SIMT_ASAN_UNPOISON(p, n) ((void)0)
+#endif
+
 // ---- keywords
 #define __global__
 #define __device__
@@ -188,7 +200,11 @@ inline bool run_cta(unsigned nthreads, size_t smem_bytes) {
     State& s = S();
     if (!s.smem || smem_bytes > SMEM_MAX) fatal("shared memory not set up or launch asks for more than 227 KB");
     s.smem_size = smem_bytes;
+    SIMT_ASAN_UNPOISON(s.smem, SMEM_MAX + 64);
     memset(s.smem, 0xFF, SMEM_MAX + 64);
+    // the scratch tail [SMEM_MAX, SMEM_MAX + 64) stays addressable: smem_ptr() redirects a faulting
+    // access there and counts it, which the tests assert on
+    SIMT_ASAN_POISON(s.smem + smem_bytes, SMEM_MAX - smem_bytes);
     s.bars.clear();
     s.tma.clear();
     s.bar_count = 0;
@@ -235,6 +251,7 @@ inline bool run_cta(unsigned nthreads, size_t smem_bytes) {
             fprintf(stderr, "simt: mbarrier @%u expected %d pending %d tx %lld phase %u\n", kv.first - SMEM_BASE, kv.second.expected, kv.second.pending, kv.second.tx, kv.second.phase);
     }
     s.fibers.clear();
+    SIMT_ASAN_UNPOISON(s.smem, SMEM_MAX + 64);
     return live == 0;
 }
 

@@ -7,6 +7,7 @@
 //       -Ipaper_1901_02492_b200/csrc -DKBMOD_SIMT_EMUL='"simt_ptx.h"' tests/hostlogic/staged_simt.cpp
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <devmem.h>
 
 namespace kbmod {
 alignas(1024) unsigned char smem_raw[simt::SMEM_MAX + 64];
@@ -38,13 +39,20 @@ int simt_search_staged(const float* psiphi, const double* times, int N, int H, i
     DtTable dt;
     for (int i = 0; i < KBMOD_MAX_IMAGES; ++i) dt.dt[i] = 0.0f;
     for (int i = 0; i < N; ++i) dt.dt[i] = (float)(times[i] - times[0]);
-    kbmod_result out{vel_idx, n_obs, psi, phi, nu, alpha};
-    std::vector<unsigned char> plan(staged_plan_bytes(N, V) + 256), enc(staged_enc_bytes(N, H, W) + 256);
-    unsigned char* encp = enc.data() + ((256 - ((uintptr_t)enc.data() & 255)) & 255);
-    int status = 0;
-    const int rc = launch_search_staged(reinterpret_cast<const float2*>(psiphi), dt, N, H, W, vel_grid, V, K, min_obs,
-                                        out, plan.data(), reinterpret_cast<const float2*>(vel_grid),
-                                        reinterpret_cast<float2*>(encp), &status, nullptr);
+    // every buffer the kernels see is its own heap block of exactly the size the product gives them
+    // (devmem.h): inputs copied in, result planes copied back
+    const size_t npix = (size_t)N * H * W, nres = (size_t)H * W * K;
+    simt::DevBuf d_pp(psiphi, npix * 8), d_vel(vel_grid, (size_t)V * 8);
+    simt::DevBuf d_plan(staged_plan_bytes(N, V)), d_enc(staged_enc_bytes(N, H, W)), d_status(sizeof(int));
+    simt::DevBuf d_vi(nres * 4), d_no(nres * 4), d_psi(nres * 4), d_phi(nres * 4), d_nu(nres * 4), d_al(nres * 4);
+    kbmod_result out{d_vi.as<int32_t>(), d_no.as<int32_t>(), d_psi.as<float>(), d_phi.as<float>(),
+                     d_nu.as<float>(), d_al.as<float>()};
+    const int rc = launch_search_staged(d_pp.as<const float2>(), dt, N, H, W, vel_grid, V, K, min_obs,
+                                        out, d_plan.p, d_vel.as<const float2>(), d_enc.as<float2>(),
+                                        d_status.as<int>(), nullptr);
+    d_vi.copy_to(vel_idx); d_no.copy_to(n_obs); d_psi.copy_to(psi); d_phi.copy_to(phi); d_nu.copy_to(nu);
+    d_al.copy_to(alpha);
+    const int status = *d_status.as<int>();
     stats[0] = s.smem_faults; stats[1] = s.tma_loads; stats[2] = s.tma_faults; stats[3] = s.launches;
     stats[4] = status; stats[5] = 0;
     return rc;

@@ -7,6 +7,7 @@
 //       -Ipaper_1901_02492_b200/csrc -DKBMOD_SIMT_EMUL=1 tests/hostlogic/tiled_simt.cpp
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <devmem.h>
 
 namespace kbmod {
 alignas(1024) unsigned char smem_raw[simt::SMEM_MAX + 64];
@@ -33,14 +34,39 @@ int simt_search_tiled(const float* psiphi, const double* times, int N, int H, in
     DtTable dt;
     for (int i = 0; i < KBMOD_MAX_IMAGES; ++i) dt.dt[i] = 0.0f;
     for (int i = 0; i < N; ++i) dt.dt[i] = (float)(times[i] - times[0]);
-    kbmod_result out{vel_idx, n_obs, psi, phi, nu, alpha};
-    std::vector<unsigned char> plan(tiled_plan_bytes(N, V, K) + 256), enc((size_t)N * H * W * 8 + 512);
-    unsigned char* encp = enc.data() + ((256 - ((uintptr_t)enc.data() & 255)) & 255);
-    const int rc = launch_search_tiled(reinterpret_cast<const float2*>(psiphi), dt, N, H, W, vel_grid, V, K, min_obs,
-                                       out, plan.data(), reinterpret_cast<const float2*>(vel_grid),
-                                       reinterpret_cast<float2*>(encp), queued != 0, nullptr);
+    // every buffer the kernels see is its own heap block of exactly the size the product gives them
+    // (devmem.h): inputs copied in, result planes copied back
+    const size_t npix = (size_t)N * H * W, nres = (size_t)H * W * K;
+    simt::DevBuf d_pp(psiphi, npix * 8), d_vel(vel_grid, (size_t)V * 8);
+    simt::DevBuf d_plan(tiled_plan_bytes(N, V, K)), d_enc(npix * 8);
+    simt::DevBuf d_vi(nres * 4), d_no(nres * 4), d_psi(nres * 4), d_phi(nres * 4), d_nu(nres * 4), d_al(nres * 4);
+    kbmod_result out{d_vi.as<int32_t>(), d_no.as<int32_t>(), d_psi.as<float>(), d_phi.as<float>(),
+                     d_nu.as<float>(), d_al.as<float>()};
+    const int rc = launch_search_tiled(d_pp.as<const float2>(), dt, N, H, W, vel_grid, V, K, min_obs,
+                                       out, d_plan.p, d_vel.as<const float2>(), d_enc.as<float2>(), queued != 0,
+                                       nullptr);
+    d_vi.copy_to(vel_idx); d_no.copy_to(n_obs); d_psi.copy_to(psi); d_phi.copy_to(phi); d_nu.copy_to(nu);
+    d_al.copy_to(alpha);
     stats[0] = s.smem_faults; stats[1] = 0; stats[2] = 0; stats[3] = s.launches; stats[4] = 0;
     return rc;
+}
+
+// launch_search_tiled's own size limits (int16 shift encoding, int32 element offsets): the launch
+// must refuse, before touching any buffer, a stack whose (N+1)*H*W element offsets do not fit int32
+int simt_tiled_limits(int N, int H, int W, int V, int K) {
+    using namespace kbmod;
+    DtTable dt;
+    for (int i = 0; i < KBMOD_MAX_IMAGES; ++i) dt.dt[i] = (float)i;
+    std::vector<float> vel((size_t)2 * V, 1.0f);
+    kbmod_result out{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    return launch_search_tiled(nullptr, dt, N, H, W, vel.data(), V, K, 1, out, nullptr, nullptr, nullptr, true, nullptr);
+}
+
+// Detector self-test: reads the element `past` elements beyond a 64-byte emulated device buffer
+// through __ldg.  past = 0 is legal; past = 1 must abort under AddressSanitizer.
+unsigned long long simt_selftest_ldg_past_end(int past) {
+    simt::DevBuf b(64);
+    return __ldg(b.as<const unsigned long long>() + 7 + past);
 }
 
 }  // extern "C"

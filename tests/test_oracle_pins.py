@@ -179,6 +179,12 @@ def test_p4_brute_force_tiny(orc, seed):
         assert np.isneginf(res["nu"][~real]).all()
         for k in ("psi", "phi", "alpha", "n_obs"):
             assert (res[k][~real] == 0).all()
+        if mode == orc.MODE_F32SEQ:
+            # the bit-level definition of f32seq (Q18; Eq.24-25): binary32 adds in
+            # image order, then correctly rounded sqrt and divisions -- a reversed or pairwise order,
+            # or a double accumulator rounded once, fails this on the random stacks
+            for k in ("psi", "phi", "nu", "alpha"):
+                assert (res[k].view(np.int32) == ref[k + "32"].view(np.int32)).all(), k
     assert (~(ref["vel_idx"] >= 0)).any() and (ref["vel_idx"] >= 0).any()
 
 

@@ -23,6 +23,7 @@ import numpy as np
 import pytest
 
 from paper_1901_02492_b200 import synth
+from tests import simt_build
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HL = os.path.join(ROOT, "tests", "hostlogic")
@@ -32,23 +33,9 @@ CSRC = os.path.join(ROOT, "paper_1901_02492_b200", "csrc")
 PLANES = ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")
 
 
-def _stale():
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    deps = [SRC, os.path.join(ROOT, "include", "kbmod_b200.h")]
-    deps += [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    deps += [os.path.join(HL, "simt", f) for f in os.listdir(os.path.join(HL, "simt"))]
-    return any(os.path.getmtime(d) > t for d in deps)
-
-
 @pytest.fixture(scope="module")
 def sim():
-    if _stale():
-        subprocess.run(["g++", "-O1", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC",
-                        "-I", os.path.join(HL, "simt"), "-I", os.path.join(ROOT, "include"), "-I", CSRC,
-                        '-DKBMOD_SIMT_EMUL="simt_ptx.h"', SRC, "-o", LIB], check=True)
-    return ctypes.CDLL(LIB)
+    return simt_build.load("staged_simt", '"simt_ptx.h"')
 
 
 def run_sim(sim, pp, times, vel, K, min_obs, order=0, seed=1, sms=3, tma_delay=0):
@@ -176,6 +163,24 @@ def test_degenerate_shapes(sim, orc):
     rc, out, stats = run_sim(sim, pp, np.arange(4.0), vel[:9], 4, 1)
     assert_exact(out, ref, stats, rc)
     assert (out["vel_idx"] == -1).all()
+
+
+def test_limit_cases(sim, orc):
+    """Image sizes around the 64 x 30 tile (one short, exact, one over; one row, one column) and
+    shifts at the edge of the int16 encoding (|v*dt| around SH_LIMIT = 30000, both signs)."""
+    vel = synth.velocity_grid(3, 3, -math.pi, math.pi, 1.0, 30.0)
+    for H, W in ((29, 63), (30, 64), (31, 65), (1, 129), (61, 1), (60, 128)):
+        pp = synth.random_psiphi(4, H, W, seed=H * 1000 + W, invalid_frac=0.1)
+        times = np.array([0.0, 0.4, 1.0, 1.7])
+        rc, out, stats = run_sim(sim, pp, times, vel, 4, 2, order=2, seed=H, sms=2, tma_delay=7)
+        assert_exact(out, orc.search(pp, times, vel, 4, 2), stats, rc)
+    pp = synth.random_psiphi(3, 40, 70, seed=9, invalid_frac=0.0)
+    big = np.array([[29999.4, 0.0], [-29999.4, 0.0], [0.0, 29999.4], [0.0, -29999.4], [30000.5, 0.0],
+                    [-30000.5, 29999.4], [29999.6, -29999.6], [30000.4, 30000.4], [1.0, 1.0], [15999.7, -15999.7],
+                    [3e38, 0.0], [-3e38, -3e38]], np.float32)
+    times = np.array([0.0, 1.0, 2.0])
+    rc, out, stats = run_sim(sim, pp, times, big, 4, 1, order=1, sms=3)
+    assert_exact(out, orc.search(pp, times, big, 4, 1), stats, rc)
 
 
 def test_image_count_variants(sim, orc):

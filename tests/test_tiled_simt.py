@@ -16,6 +16,7 @@ import numpy as np
 import pytest
 
 from paper_1901_02492_b200 import synth
+from tests import simt_build
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HL = os.path.join(ROOT, "tests", "hostlogic")
@@ -26,23 +27,9 @@ PLANES = ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")
 TILED, QUEUED = 0, 1
 
 
-def _stale():
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    deps = [SRC, os.path.join(ROOT, "include", "kbmod_b200.h")]
-    deps += [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    deps += [os.path.join(HL, "simt", f) for f in os.listdir(os.path.join(HL, "simt"))]
-    return any(os.path.getmtime(d) > t for d in deps)
-
-
 @pytest.fixture(scope="module")
 def sim():
-    if _stale():
-        subprocess.run(["g++", "-O1", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC",
-                        "-I", os.path.join(HL, "simt"), "-I", os.path.join(ROOT, "include"), "-I", CSRC,
-                        "-DKBMOD_SIMT_EMUL=1", SRC, "-o", LIB], check=True)
-    return ctypes.CDLL(LIB)
+    return simt_build.load("tiled_simt", '1')
 
 
 def run_sim(sim, pp, times, vel, K, min_obs, queued, order=0, seed=1):
@@ -146,6 +133,42 @@ def test_queued_image_count_variants(sim, orc):
         times = np.sort(rng.uniform(0.0, 5.0, N))
         vel = synth.velocity_grid(6, 4, -math.pi / 2, math.pi / 2, 1.0, 9.0)
         assert_exact(run_sim(sim, pp, times, vel, 8, mo, QUEUED, order=2, seed=N), orc.search(pp, times, vel, 8, mo))
+
+
+@pytest.mark.parametrize("queued", [TILED, QUEUED])
+def test_limit_cases(sim, orc, queued):
+    """The limits the GPU tests do not reach: image sizes around the 64 x 32 tile (one short, exact,
+    one over; one row, one column), shifts at the edge of the int16 shift encoding (|v*dt| around
+    SH_LIMIT = 32000: proven, skipped, and both signs), and blocks whose clean velocities are
+    completed with benign padding while the tile touches every image corner."""
+    rng = np.random.default_rng(5)
+    vel = synth.velocity_grid(3, 3, -math.pi, math.pi, 1.0, 30.0)
+    for H, W in ((31, 63), (32, 64), (33, 65), (1, 129), (70, 1), (64, 128)):
+        pp = synth.random_psiphi(4, H, W, seed=H * 1000 + W, invalid_frac=0.1)
+        times = np.array([0.0, 0.4, 1.0, 1.7])
+        assert_exact(run_sim(sim, pp, times, vel, 4, 2, queued, order=2, seed=H), orc.search(pp, times, vel, 4, 2))
+    # shifts at the limits of the encoding: +-31999.4 is a proven shift, 32000.5 is skipped; the image
+    # is tiny, so every such window is far outside (no sample may be fetched, n_obs counts image 0 only)
+    pp = synth.random_psiphi(3, 40, 70, seed=9, invalid_frac=0.0)
+    big = np.array([[31999.4, 0.0], [-31999.4, 0.0], [0.0, 31999.4], [0.0, -31999.4], [32000.5, 0.0],
+                    [-32000.5, 31999.4], [29999.6, -29999.6], [30000.4, 30000.4], [1.0, 1.0], [15999.7, -15999.7],
+                    [3e38, 0.0], [-3e38, -3e38]], np.float32)
+    times = np.array([0.0, 1.0, 2.0])
+    assert_exact(run_sim(sim, pp, times, big, 4, 1, queued, order=1), orc.search(pp, times, big, 4, 1))
+    # half-integer velocities inside chunks of clean ones (kernel 4: benign padding next to the corners)
+    vel = synth.velocity_grid(4, 5, -math.pi, math.pi, 2.0, 24.0)
+    vel[[1, 6, 7, 13]] = np.array([[10.5, 3.0], [-2.5, -7.5], [0.5, 0.5], [63.5, 31.5]], np.float32)
+    pp = synth.random_psiphi(5, 33, 66, seed=12, invalid_frac=0.2)
+    times = np.array([0.0, 1.0, 2.0, 3.0, 1.0])
+    assert_exact(run_sim(sim, pp, times, vel, 8, 2, queued, order=2, seed=3), orc.search(pp, times, vel, 8, 2))
+
+
+def test_limit_on_stack_size_is_refused_before_any_access(sim):
+    """(N+1)*H*W + SH_LIMIT*(W+1) must stay below 2^31 (int32 element offsets): the launch returns
+    KBMOD_ERR_UNSUPPORTED (-6) without touching a buffer (all pointers are NULL here)."""
+    assert sim.simt_tiled_limits(15, 11000, 11000, 8, 8) == -6        # 16 * 1.21e8 = 1.9e9 + 3.5e8 > 2^31
+    assert sim.simt_tiled_limits(3, 30001, 100, 8, 8) == -6           # beyond the int16 shift range
+    assert sim.simt_tiled_limits(64, 8192, 8192, 8, 8) == -6          # 65 * 2^26 > 2^31
 
 
 def random_case(rng):
