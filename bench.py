@@ -10,11 +10,12 @@ of the result planes inside the timed region).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3] [--kernel 0]
 
---kernel 0 (default): the library's default search kernel, the one the GPU test suite validates
-against the oracle; the same kernel every run.  --kernel k forces kernel k.  --kernel -1 (explicit
-opt-in, never the driver's run): a child process runs the workload with the default kernel and with
-candidate 4, compares all six result planes bit for bit on the device and times both; the candidate
-is timed only if identical AND faster ("kernel_selection" in the line).
+--kernel 0 (default): the library's default search kernel (KBMOD_KERNEL_AUTO), the one the GPU test
+suite validates against the oracle; the same kernel every run.  --kernel k (1 direct, 2 tiled,
+3 TMA-staged, 4 tiled + queued top-K) times that kernel instead; 3 and 4 are opt-in until they have
+passed the GPU suite on hardware.  The kernel and its knobs travel in
+kbmod_search_options; the host plan (kbmod_plan: it depends on times / grid / shape only) is built
+once before the timed region, as a survey pipeline searching many stacks of one cadence would.
 
 N > 1 (torchrun): every rank searches its own independent stack (the survey's fields/CCDs are
 independent searches) -- weak scaling, no data-path collective.
@@ -41,10 +42,31 @@ UNIT = "trajectory-evals/s"
 SM_COUNT = 148
 LDS_BYTES_PER_CLK_PER_SM = 128          # shared-memory crossbar (B300_MICROARCH.md "LDS/STS")
 SAMPLE_BYTES = 8                        # one float2 (psi, phi) per trajectory-eval
-# dram__bytes_read.sum + dram__bytes_write.sum of the search kernel, one launch at config 3, from
-# the committed `ncu --set full` captures (profiles/r01_v1_direct.md, profiles/r01_v2_tiled.md);
-# keyed by the kernel kbmod_set_search_kernel selects (0 = automatic = the tiled kernel).
-NCU_DRAM_BYTES_CONFIG3 = {1: 666.6e9 + 3.67e9, 0: 218.9e9 + 3.23e9, 2: 218.9e9 + 3.23e9}
+KERNEL_NAMES = {0: "search_tiled_kernel (automatic)", 1: "search_direct_kernel", 2: "search_tiled_kernel",
+                3: "search_staged_kernel", 4: "search_tiledq_kernel"}
+
+
+def last_capture(kernel):
+    """The last committed `ncu --set full` capture of this search kernel at the bench workload
+    (profiles/ncu_captures.csv, hand-copied from the summaries it cites).  It describes the commit
+    it names, not this run: it is reported beside the roofline, never as `traffic`."""
+    import csv
+    p = os.path.join(ROOT, "profiles", "ncu_captures.csv")
+    if not os.path.exists(p):
+        return None
+    name = KERNEL_NAMES.get(kernel, "").split(" ")[0]
+    for row in csv.DictReader(open(p)):
+        if row["kernel"] == name:
+            out = {}
+            for k, v in row.items():
+                try:
+                    out[k] = float(v) if k not in ("kernel", "commit", "source", "note") else v
+                except ValueError:
+                    out[k] = v or None
+            out["l2_to_sm_bytes_per_sample_byte"] = (out["l2_to_l1_bytes"] / (15 * 4096 * 4096 * 640 * 8.0)
+                                                     if out.get("l2_to_l1_bytes") else None)
+            return out
+    return None
 
 
 def load_peaks():
@@ -171,83 +193,6 @@ def config_dict(cfg, args):
 
 
 # ----------------------------------------------------------------------------------------------
-# kernel selection by measurement (child process: its own CUDA context)
-# ----------------------------------------------------------------------------------------------
-CANDIDATE_KERNEL = 4
-GROUPW_SWEEP = (8, 4, 16, 2)            # KBMOD_TILED_GROUPW values tried for the candidate (8 = its default)
-KERNEL_NAMES = {0: "search_tiled_kernel (automatic)", 1: "search_direct_kernel", 2: "search_tiled_kernel",
-                3: "search_staged_kernel", 4: "search_tiledq_kernel"}
-
-
-def probe_child(args, cfg, local_rank):
-    """Child mode (--probe): default kernel vs candidate on this workload; prints one JSON line."""
-    import torch
-    from paper_1901_02492_b200 import binding, build
-    build.build()
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    st = synth.make_stack(cfg, seed=args.probe_seed)
-    N, H, W, V, K = cfg.N, cfg.H, cfg.W, cfg.V, cfg.K
-    to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
-    psiphi = binding.make_psi_phi(to(st.sci), to(st.var), to(st.mask), st.psf)
-    ws = torch.empty(binding.search_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
-    def run(which, out):
-        binding.set_search_kernel(which)
-        ts = []
-        for _ in range(3):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            binding.search(psiphi, st.times, st.vel_grid, K, cfg.min_obs, out=out, workspace=ws)
-            b.record()
-            binding.search_status(ws)
-            ts.append(a.elapsed_time(b))
-        return float(np.median(ts))
-
-    ref = binding.alloc_result(H, W, K, dev)
-    ms_default = run(0, ref)
-    # the candidate under each tile-rasterisation width (results do not depend on it; speed may)
-    sweep, best = {}, None
-    out = binding.alloc_result(H, W, K, dev)
-    for gw in GROUPW_SWEEP:
-        os.environ["KBMOD_TILED_GROUPW"] = str(gw)
-        for v in out.values():
-            v.zero_()
-        ms = run(CANDIDATE_KERNEL, out)
-        same = all(torch.equal(ref[k].view(torch.int32), out[k].view(torch.int32)) for k in ref)
-        sweep[str(gw)] = {"ms": ms, "identical": bool(same)}
-        if same and (best is None or ms < sweep[str(best)]["ms"]):
-            best = gw
-    print(json.dumps({"probe": True, "identical": best is not None, "ms_default": ms_default,
-                      "ms_candidate": sweep[str(best)]["ms"] if best is not None else None,
-                      "groupw": best, "groupw_sweep": sweep}))
-
-
-def select_kernel(args, seed, local_rank):
-    """Parent: returns (kernel id, report dict)."""
-    cmd = [sys.executable, os.path.abspath(__file__), "--probe", "--probe-seed", str(seed),
-           "--config", str(args.config), "--rows", str(args.rows)]
-    env = dict(os.environ, LOCAL_RANK=str(local_rank), WORLD_SIZE="1", RANK="0")
-    rep = {"default": KERNEL_NAMES[0], "candidate": KERNEL_NAMES[CANDIDATE_KERNEL]}
-    try:
-        cp = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env=env)
-        lines = [l for l in cp.stdout.splitlines() if l.startswith('{"probe"')]
-        if cp.returncode != 0 or not lines:
-            rep["error"] = f"probe exited {cp.returncode}: {cp.stderr.strip()[-200:]}"
-            return 0, rep
-        rep.update(json.loads(lines[-1]))
-        use = bool(rep["identical"]) and rep["ms_candidate"] < rep["ms_default"]
-        if use and rep.get("groupw"):
-            os.environ["KBMOD_TILED_GROUPW"] = str(rep["groupw"])      # read by the library at each launch
-        rep["selected"] = KERNEL_NAMES[CANDIDATE_KERNEL if use else 0]
-        rep["rule"] = ("candidate only if all six result planes are bit-identical to the default kernel's and it is "
-                       "faster; its tile-rasterisation width is the fastest identical one of the sweep")
-        return (CANDIDATE_KERNEL if use else 0), rep
-    except Exception as exc:
-        rep["error"] = f"{type(exc).__name__}: {exc}"[:200]
-        return 0, rep
-
-
-# ----------------------------------------------------------------------------------------------
 # GPU arm
 # ----------------------------------------------------------------------------------------------
 def run_gpu(args, cfg, st, rank, world, local_rank):
@@ -260,16 +205,11 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
         raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    selection = None
     kernel = args.kernel
-    if kernel < 0:
-        kernel, selection = select_kernel(args, shard.rank_seed(cfg.seed, rank), local_rank)
-        if world > 1:                       # every rank times the same kernel: the candidate only if all agree
-            t = torch.tensor([kernel], device=dev, dtype=torch.int32)
-            dist.all_reduce(t, op=dist.ReduceOp.MIN)
-            kernel = int(t.item())
-    binding.set_search_kernel(kernel)
     N, H, W, V, K = cfg.N, cfg.H, cfg.W, cfg.V, cfg.K
+    # the host plan depends on (times, grid, shape, K, options) only: built once, outside the timed region
+    plan = binding.Plan(st.times, N, H, W, st.vel_grid, K, kernel=kernel, tile_group_w=args.group_w,
+                        staged_geom=args.staged_geom)
 
     # pinned host inputs and outputs (for e2e), resident device copies (for value)
     h_sci = torch.from_numpy(st.sci).pin_memory()
@@ -284,14 +224,14 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
 
     def step_resident():
         binding.make_psi_phi(d_sci, d_var, d_mask, st.psf, out=psiphi)
-        binding.search(psiphi, st.times, st.vel_grid, K, cfg.min_obs, out=out, workspace=ws)
+        binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan)
 
     def step_e2e():
         e_sci.copy_(h_sci, non_blocking=True)
         e_var.copy_(h_var, non_blocking=True)
         e_mask.copy_(h_mask, non_blocking=True)
         binding.make_psi_phi(e_sci, e_var, e_mask, st.psf, out=psiphi)
-        binding.search(psiphi, st.times, st.vel_grid, K, cfg.min_obs, out=out, workspace=ws)
+        binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan)
         for k in out:
             h_out[k].copy_(out[k], non_blocking=True)
 
@@ -337,8 +277,8 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
         return float(np.median(ts))
     reps = max(3, min(args.steps, 10))
     ms_psiphi = phase(lambda: binding.make_psi_phi(d_sci, d_var, d_mask, st.psf, out=psiphi), reps)
-    ms_search = phase(lambda: binding.search(psiphi, st.times, st.vel_grid, K, cfg.min_obs,
-                                             out=out, workspace=ws), reps)
+    ms_search = phase(lambda: binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws,
+                                             plan=plan), reps)
 
     binding.search_status(ws)
     step_e2e()
@@ -353,7 +293,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
             raise RuntimeError("measured at N=1 only")
         ws_h = torch.empty(binding.search_host_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
         run_h = lambda: binding.search_host(h_sci, h_var, h_mask, st.psf, st.times, st.vel_grid, K,
-                                            cfg.min_obs, h_out, ws_h)
+                                            cfg.min_obs, h_out, ws_h, kernel=kernel)
         run_h()
         binding.search_status(ws_h)
         same = all(torch.equal(h_out[k], out[k].cpu()) or k in ("nu", "alpha", "psi", "phi") and
@@ -403,9 +343,10 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
                         "trajectories_per_s": cfg.trajectories / (ms_search * 1e-3)},
         "roofline": {"bound": "smem", "achieved": achieved, "peak": lsu_peak, "unit": "GB/s",
                      "frac": achieved / lsu_peak,
-                     "traffic": (NCU_DRAM_BYTES_CONFIG3.get(kernel)
-                                 if args.config == 3 and not args.rows else None),
-                     "traffic_source": "profiles/ (ncu --set full of an earlier run of this kernel)",
+                     # dram bytes of THIS build's kernel need an ncu capture of this commit; none exists
+                     # until one is taken (profiles/), so none is claimed
+                     "traffic": None,
+                     "last_capture": (last_capture(kernel) if args.config == 3 and not args.rows else None),
                      "kernel": f"kbmod_search -> {KERNEL_NAMES.get(kernel, kernel)}",
                      "peak_source": f"148 SM x 128 B/clk x {sm_max_mhz:.0f} MHz ({peak_src} max "
                                     "SM clock); north_star roofline = slower of HBM and LSU",
@@ -418,7 +359,8 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
         "e2e_binding_copies": e2e_binding,
         "e2e_host_abi": host_abi,
         "search_kernel": KERNEL_NAMES.get(kernel, str(kernel)),
-        "kernel_selection": selection if selection is not None else {"selected": KERNEL_NAMES.get(kernel), "rule": "--kernel given"},
+        "search_options": {"kernel": kernel, "tile_group_w": args.group_w, "staged_geom": args.staged_geom,
+                           "plan": "kbmod_plan built once before the timed region"},
     }
     if world == 1 and not args.no_cpu:
         import oracle
@@ -441,12 +383,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--rows", type=int, default=0, help="override H (debug only)")
-    ap.add_argument("--kernel", type=int, default=0,
-                    help="0 library default (the kernel the GPU test suite validates; the default), 1 direct, "
-                         "2 tiled, 3 TMA-staged, 4 tiled + queued top-K, -1 choose by measurement between the "
-                         "default and candidate 4 in a child process (explicit opt-in only)")
-    ap.add_argument("--probe", action="store_true", help="child mode of --kernel -1 (internal)")
-    ap.add_argument("--probe-seed", type=int, default=0, help="stack seed of the probe (internal)")
+    ap.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2, 3, 4],
+                    help="0 library default (the kernel the GPU test suite validates), 1 direct, 2 tiled, "
+                         "3 TMA-staged, 4 tiled + queued top-K (3 and 4: opt-in, see DESIGN.md section 8)")
+    ap.add_argument("--group-w", type=int, default=0, help="kbmod_search_options.tile_group_w (0 = default)")
+    ap.add_argument("--staged-geom", type=int, default=0, help="kbmod_search_options.staged_geom (kernel 3)")
     ap.add_argument("--ref-rows", type=int, default=256, help="start rows per oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
@@ -455,10 +396,6 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     cfg = workload(args)
-
-    if args.probe:
-        probe_child(args, cfg, local_rank)
-        return
 
     if args.impl == "reference":
         if rank != 0:

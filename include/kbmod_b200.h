@@ -5,7 +5,9 @@
  * arXiv:1901.02492; citations below are PAPER.md line numbers "P:<line>"):
  *   1. kbmod_make_psi_phi : per-image likelihood images Psi_i, Phi_i   (Eq.19-20)
  *   2. kbmod_search       : exhaustive linear-trajectory search        (Eq.24-27)
- * plus a test hook (kbmod_eval_trajectories) and small utilities.
+ * plus the band / options / prebuilt-plan forms of the search (kbmod_search_rows,
+ * kbmod_plan_create, kbmod_search_planned), a test hook (kbmod_eval_trajectories) and small
+ * utilities.
  *
  * Conventions
  *   - Plain C, no torch / C++ types.  Pointers are DEVICE pointers unless marked HOST.
@@ -18,6 +20,13 @@
  *     before any launch; asynchronous faults surface at the caller's next synchronisation.
  *   - There is no CPU fallback: without a CUDA device every compute call returns
  *     KBMOD_ERR_CUDA.
+ *   - No environment variable and no process-wide setting influences any call: what selects a
+ *     kernel or tunes it is an argument (kbmod_search_options).  Calls on distinct streams with
+ *     distinct workspaces are independent and thread-safe.
+ *   - Deviation from the two-call signature of the problem statement, which lists vel_grid among
+ *     the device arrays: vel_grid (and times) are HOST arrays here, because the library derives
+ *     its per-(velocity, image) integer-shift plan from them on the host before any launch; it
+ *     keeps its own device copy in the workspace.
  */
 #ifndef KBMOD_B200_H
 #define KBMOD_B200_H
@@ -82,6 +91,25 @@ int kbmod_make_psi_phi(const float* sci, const float* var, const uint8_t* mask,
                        const float* psf, int N, int H, int W, int P,
                        float* psiphi, void* stream);
 
+/* Which search kernel runs (kbmod_search_options.kernel).  All return bit-identical results. */
+enum {
+    KBMOD_KERNEL_AUTO = 0,          /* the tiled kernel where the shape fits, else the direct-gather kernel */
+    KBMOD_KERNEL_DIRECT = 1,        /* literal S3 per sample, global loads, any shape */
+    KBMOD_KERNEL_TILED = 2,         /* host-proven integer shifts, global loads through L1 */
+    KBMOD_KERNEL_STAGED = 3,        /* TMA-staged shared-memory windows, persistent CTAs */
+    KBMOD_KERNEL_TILED_QUEUED = 4   /* the gathers of 2 with queue-compacted top-K */
+};
+
+/* Options of a search.  Zero-initialise; every field's 0 is its default; NULL = all defaults.
+ * With kernel 2, 3 or 4 the call returns KBMOD_ERR_UNSUPPORTED if the shape does not fit it. */
+typedef struct {
+    int32_t struct_size;    /* 0 or sizeof(kbmod_search_options) */
+    int32_t kernel;         /* KBMOD_KERNEL_* */
+    int32_t tile_group_w;   /* kernels 2, 4: tile columns per rasterisation group, 1..256; 0 = default.
+                               Changes which CTA takes which tile, never the results */
+    int32_t staged_geom;    /* kernel 3: shared-memory ring geometry 0..6 (csrc/search_staged.cu) */
+} kbmod_search_options;
+
 /*
  * Exhaustive search (Eq.27).  For every start pixel (x0,y0) of image 0
  * and every velocity j of vel_grid:
@@ -107,6 +135,41 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
                  const float* vel_grid, int V, int K, int min_obs,
                  const kbmod_result* out, void* workspace, size_t workspace_bytes,
                  void* stream);
+
+/*
+ * kbmod_search restricted to the start rows y_begin <= y0 < y_end (0 <= y_begin <= y_end <= H), with
+ * options.  Every evaluation is independent and top-K never crosses start pixels, so bands
+ * of one replicated stack searched on different GPUs concatenate to the full search (row-band
+ * sharding).  Trajectories still sample the whole images.
+ *   out       : planes of the BAND only, each [(y_end - y_begin)][W][K]; row 0 = start row y_begin
+ *   options   : HOST, may be NULL
+ * Other arguments as kbmod_search (the workspace size does not depend on the band).
+ */
+int kbmod_search_rows(const float* psiphi, const double* times, int N, int H, int W,
+                      const float* vel_grid, int V, int K, int min_obs, int y_begin, int y_end,
+                      const kbmod_result* out, void* workspace, size_t workspace_bytes,
+                      const kbmod_search_options* options, void* stream);
+
+/*
+ * The host plan of a search, built once and reused.  Everything kbmod_search derives from (times,
+ * velocity grid, image shape, K, options) before it looks at a pixel -- the velocity processing
+ * order, the proof that one integer shift per (velocity, image) reproduces S3 for every start pixel
+ * (P:203), the staged kernel's box stream -- lives in an opaque HOST object, so repeated
+ * searches of stacks taken at the same epochs with the same grid do not rebuild it.
+ *   kbmod_plan_create    : argument checks as kbmod_search; *plan receives the object.  No CUDA call.
+ *   kbmod_plan_kernel    : the KBMOD_KERNEL_* the plan resolved to (AUTO never remains)
+ *   kbmod_search_planned : kbmod_search_rows with the plan's times / grid / shape / K / options
+ *   kbmod_plan_destroy   : frees it (NULL is allowed); the plan may be destroyed as soon as the
+ *                          searches using it have returned
+ * A plan is immutable: any number of searches on any streams may share it concurrently.
+ */
+typedef struct kbmod_plan kbmod_plan;
+int kbmod_plan_create(const double* times, int N, int H, int W, const float* vel_grid, int V, int K,
+                      const kbmod_search_options* options, kbmod_plan** plan);
+int kbmod_plan_kernel(const kbmod_plan* plan);
+int kbmod_search_planned(const kbmod_plan* plan, const float* psiphi, int min_obs, int y_begin, int y_end,
+                         const kbmod_result* out, void* workspace, size_t workspace_bytes, void* stream);
+void kbmod_plan_destroy(kbmod_plan* plan);
 
 /* Completion status of the last kbmod_search that used this workspace.  SYNCHRONISES the stream
  * (the one call of the library that does).  KBMOD_OK, or KBMOD_ERR_TIMEOUT if a warp of the
@@ -136,11 +199,13 @@ int kbmod_search_split(const float* psi, const float* phi, const double* times, 
  *   workspace: DEVICE scratch of at least kbmod_search_host_workspace(N,H,W,V,K) bytes, 256-byte
  *              aligned (holds the device copies of the inputs, psi/phi, the result planes and
  *              the search workspace); kbmod_search_status(workspace, stream) works on it too
+ *   options  : HOST, may be NULL
+ * Every argument error of both stages is reported before the first copy is enqueued.
  */
 int kbmod_search_host(const float* sci, const float* var, const uint8_t* mask, const float* psf,
                       const double* times, int N, int H, int W, int P, const float* vel_grid, int V,
                       int K, int min_obs, const kbmod_result* out, void* workspace,
-                      size_t workspace_bytes, void* stream);
+                      size_t workspace_bytes, const kbmod_search_options* options, void* stream);
 size_t kbmod_search_host_workspace(int N, int H, int W, int V, int K);
 
 /*
@@ -155,21 +220,12 @@ int kbmod_eval_trajectories(const float* psiphi, const double* times, int N, int
                             float* Psi, float* Phi, int32_t* n_obs, int32_t* ixiy,
                             void* stream);
 
-/* Selects the search kernel: 0 = automatic (default: the tiled kernel where the shape fits, else
- * the direct-gather kernel), 1 = direct-gather kernel (global loads, any shape), 2 = tiled kernel
- * (host-proven integer shifts, global loads through L1), 3 = TMA-staged shared-memory kernel,
- * 4 = tiled kernel with queue-compacted top-K (the gathers of 2, the S5/S6 of 3).
- * With 2, 3 or 4 kbmod_search returns KBMOD_ERR_UNSUPPORTED if the shape does not fit that kernel.
- * All kernels return bit-identical results.
- * Process-wide; for tests and benchmarks. */
-int kbmod_set_search_kernel(int which);
-
 /*
  * Test hook (host only, no CUDA call): the plan the TMA-staged kernel would execute for these
  * inputs, so that its host logic -- the proof that one integer shift per (velocity, image)
  * reproduces S3 for every start pixel, the grouping of shifted windows into shared-memory boxes,
  * the per-member offsets -- can be checked against the oracle without a GPU.
- *   times, vel_grid : HOST, as for kbmod_search
+ *   times, vel_grid : HOST, as for kbmod_search;  staged_geom : as kbmod_search_options.staged_geom
  *   stream  : HOST out, nent entries of info[1] int32 each (layout: csrc/search_staged.cu)
  *   shapes  : HOST out, [nshapes][2] = (box width, box height) in samples, index = tensor-map id
  *   info    : HOST out [8] = nent, ints per entry, nshapes, tile width, tile height, velocities
@@ -177,8 +233,8 @@ int kbmod_set_search_kernel(int which);
  * Returns KBMOD_ERR_WORKSPACE (with info filled) if stream_ints / max_shapes are too small.
  */
 int kbmod_debug_staged_plan(const double* times, int N, int H, int W, const float* vel_grid, int V,
-                            int32_t* stream, size_t stream_ints, int32_t* shapes, int max_shapes,
-                            int32_t* info);
+                            int staged_geom, int32_t* stream, size_t stream_ints, int32_t* shapes,
+                            int max_shapes, int32_t* info);
 
 /* Number of kernel launches issued by this library since load (for benchmark accounting). */
 unsigned long long kbmod_launch_count(void);

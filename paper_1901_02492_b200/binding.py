@@ -17,10 +17,15 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libkbmod_b200.so")
 _lib: Optional[ctypes.CDLL] = None
 
-EXPORTS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_workspace", "kbmod_search_split",
-           "kbmod_eval_trajectories", "kbmod_set_search_kernel", "kbmod_launch_count",
-           "kbmod_status_string", "kbmod_version", "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host",
+EXPORTS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_rows", "kbmod_search_workspace",
+           "kbmod_search_split", "kbmod_plan_create", "kbmod_plan_kernel", "kbmod_search_planned",
+           "kbmod_plan_destroy", "kbmod_eval_trajectories", "kbmod_launch_count", "kbmod_status_string",
+           "kbmod_version", "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host",
            "kbmod_search_host_workspace")
+_INT_CALLS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_rows", "kbmod_search_split",
+              "kbmod_plan_create", "kbmod_plan_kernel", "kbmod_search_planned", "kbmod_eval_trajectories",
+              "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host")
+KERNEL_AUTO, KERNEL_DIRECT, KERNEL_TILED, KERNEL_STAGED, KERNEL_TILED_QUEUED = range(5)
 
 
 class KbmodError(RuntimeError):
@@ -29,6 +34,20 @@ class KbmodError(RuntimeError):
 
 class _Result(ctypes.Structure):
     _fields_ = [(n, ctypes.c_void_p) for n in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")]
+
+
+class _Options(ctypes.Structure):          # kbmod_search_options
+    _fields_ = [(n, ctypes.c_int32) for n in ("struct_size", "kernel", "tile_group_w", "staged_geom")]
+
+
+# Default kernel of THIS MODULE's calls (a Python-side convenience for tests and benchmarks; the
+# library itself has no process-wide setting: the choice travels in kbmod_search_options).
+_default_kernel = KERNEL_AUTO
+
+
+def _options(kernel=None, tile_group_w=0, staged_geom=0) -> _Options:
+    k = _default_kernel if kernel is None else int(kernel)
+    return _Options(ctypes.sizeof(_Options), k, int(tile_group_w), int(staged_geom))
 
 
 def lib() -> ctypes.CDLL:
@@ -44,11 +63,9 @@ def lib() -> ctypes.CDLL:
         L.kbmod_launch_count.restype = ctypes.c_ulonglong
         L.kbmod_status_string.restype = ctypes.c_char_p
         L.kbmod_version.restype = ctypes.c_char_p
-        for n in ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_split",
-                  "kbmod_eval_trajectories", "kbmod_set_search_kernel",
-                  "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host",
-           "kbmod_search_host_workspace"):
+        for n in _INT_CALLS:
             getattr(L, n).restype = ctypes.c_int
+        L.kbmod_plan_destroy.restype = None
         _lib = L
     return _lib
 
@@ -85,7 +102,43 @@ def launch_count() -> int:
 
 
 def set_search_kernel(which: int) -> None:
-    _check(lib().kbmod_set_search_kernel(int(which)), "kbmod_set_search_kernel")
+    """Sets the kernel this module passes in kbmod_search_options when a call names none."""
+    global _default_kernel
+    if not 0 <= int(which) <= 4:
+        raise KbmodError(f"unknown search kernel {which}")
+    _default_kernel = int(which)
+
+
+class Plan:
+    """kbmod_plan: the host plan of a search (times, velocity grid, shape, K, options), built once."""
+
+    def __init__(self, times, N: int, H: int, W: int, vel_grid, K: int, kernel=None, tile_group_w=0,
+                 staged_geom=0):
+        t = _host(times, np.float64)
+        v = _host(vel_grid, np.float32)
+        if t.shape != (N,) or v.ndim != 2 or v.shape[1] != 2:
+            raise KbmodError("times must be [N], vel_grid [V,2]")
+        self.N, self.H, self.W, self.V, self.K = int(N), int(H), int(W), int(v.shape[0]), int(K)
+        self._h = ctypes.c_void_p()
+        opt = _options(kernel, tile_group_w, staged_geom)
+        _check(lib().kbmod_plan_create(t.ctypes.data_as(ctypes.c_void_p), self.N, self.H, self.W,
+                                       v.ctypes.data_as(ctypes.c_void_p), self.V, self.K, ctypes.byref(opt),
+                                       ctypes.byref(self._h)), "kbmod_plan_create")
+
+    @property
+    def kernel(self) -> int:
+        return int(lib().kbmod_plan_kernel(self._h))
+
+    def close(self) -> None:
+        if self._h:
+            lib().kbmod_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def search_status(workspace: torch.Tensor) -> None:
@@ -95,7 +148,7 @@ def search_status(workspace: torch.Tensor) -> None:
            "kbmod_search_status")
 
 
-def debug_staged_plan(times, N: int, H: int, W: int, vel_grid):
+def debug_staged_plan(times, N: int, H: int, W: int, vel_grid, staged_geom: int = 0):
     """kbmod_debug_staged_plan (host only): returns (stream [nent, ints_per_entry] int32,
     shapes [nshapes, 2] int32, info dict)."""
     t = _host(times, np.float64)
@@ -107,7 +160,7 @@ def debug_staged_plan(times, N: int, H: int, W: int, vel_grid):
     shapes = np.zeros((4096, 2), np.int32)
     info = np.zeros(8, np.int32)
     rc = lib().kbmod_debug_staged_plan(t.ctypes.data_as(ctypes.c_void_p), N, H, W,
-                                       v.ctypes.data_as(ctypes.c_void_p), V,
+                                       v.ctypes.data_as(ctypes.c_void_p), V, int(staged_geom),
                                        stream.ctypes.data_as(ctypes.c_void_p), ctypes.c_size_t(cap),
                                        shapes.ctypes.data_as(ctypes.c_void_p), 4096,
                                        info.ctypes.data_as(ctypes.c_void_p))
@@ -149,36 +202,58 @@ def alloc_result(H: int, W: int, K: int, device) -> Dict[str, torch.Tensor]:
     return r
 
 
+def _result_struct(out: Dict[str, torch.Tensor], rows: int, W: int, K: int) -> _Result:
+    for k in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha"):
+        _dev(out[k], torch.int32 if k in ("vel_idx", "n_obs") else torch.float32, k)
+        if tuple(out[k].shape) != (rows, W, K):
+            raise KbmodError(f"result plane {k}: expected shape {(rows, W, K)}, got {tuple(out[k].shape)}")
+    return _Result(*[ctypes.c_void_p(out[k].data_ptr()) for k in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")])
+
+
 def search(psiphi: torch.Tensor, times, vel_grid, K: int, min_obs: int,
            out: Optional[Dict[str, torch.Tensor]] = None,
-           workspace: Optional[torch.Tensor] = None) -> Dict[str, torch.Tensor]:
-    """kbmod_search: psiphi [N,H,W,2] f32 cuda, times host [N] f64, vel_grid host [V,2] f32."""
+           workspace: Optional[torch.Tensor] = None, y_begin: int = 0, y_end: Optional[int] = None,
+           kernel: Optional[int] = None, tile_group_w: int = 0, staged_geom: int = 0,
+           plan: Optional[Plan] = None) -> Dict[str, torch.Tensor]:
+    """kbmod_search_rows (kbmod_search_planned when `plan` is given): psiphi [N,H,W,2] f32 cuda, times
+    host [N] f64, vel_grid host [V,2] f32.  Searches the start rows [y_begin, y_end) (default: all);
+    the result planes hold that band only, [(y_end - y_begin), W, K]."""
     N, H, W, two = psiphi.shape
     if two != 2:
         raise KbmodError("psiphi must be [N,H,W,2]")
-    times = _host(times, np.float64)
-    vel = _host(vel_grid, np.float32)
-    if times.shape != (N,) or vel.ndim != 2 or vel.shape[1] != 2:
-        raise KbmodError("times must be [N], vel_grid [V,2]")
-    V = vel.shape[0]
+    y_end = H if y_end is None else int(y_end)
+    y_begin = int(y_begin)
+    if plan is not None:
+        if (plan.N, plan.H, plan.W, plan.K) != (N, H, W, int(K)):
+            raise KbmodError("plan was built for another shape or K")
+        V = plan.V
+    else:
+        times = _host(times, np.float64)
+        vel = _host(vel_grid, np.float32)
+        if times.shape != (N,) or vel.ndim != 2 or vel.shape[1] != 2:
+            raise KbmodError("times must be [N], vel_grid [V,2]")
+        V = vel.shape[0]
+    rows = max(0, y_end - y_begin)
     if out is None:
-        out = alloc_result(H, W, K, psiphi.device)
+        out = alloc_result(rows, W, K, psiphi.device)
     need = search_workspace(N, H, W, V, K)
     own_workspace = workspace is None
     if own_workspace:
         workspace = torch.empty(need, dtype=torch.uint8, device=psiphi.device)
-    res = _Result(*[ctypes.c_void_p(out[k].data_ptr()) for k in
-                    ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")])
-    for k in ("vel_idx", "n_obs"):
-        _dev(out[k], torch.int32, k)
-    for k in ("psi", "phi", "nu", "alpha"):
-        _dev(out[k], torch.float32, k)
-    rc = lib().kbmod_search(_dev(psiphi, torch.float32, "psiphi"),
-                            times.ctypes.data_as(ctypes.c_void_p), N, H, W,
-                            vel.ctypes.data_as(ctypes.c_void_p), V, int(K), int(min_obs),
-                            ctypes.byref(res), _dev(workspace, torch.uint8, "workspace"),
-                            ctypes.c_size_t(workspace.numel()), _stream())
-    _check(rc, "kbmod_search")
+    res = _result_struct(out, rows, W, int(K))
+    if plan is not None:
+        rc = lib().kbmod_search_planned(plan._h, _dev(psiphi, torch.float32, "psiphi"), int(min_obs), y_begin,
+                                        y_end, ctypes.byref(res), _dev(workspace, torch.uint8, "workspace"),
+                                        ctypes.c_size_t(workspace.numel()), _stream())
+        _check(rc, "kbmod_search_planned")
+    else:
+        opt = _options(kernel, tile_group_w, staged_geom)
+        rc = lib().kbmod_search_rows(_dev(psiphi, torch.float32, "psiphi"),
+                                     times.ctypes.data_as(ctypes.c_void_p), N, H, W,
+                                     vel.ctypes.data_as(ctypes.c_void_p), V, int(K), int(min_obs), y_begin, y_end,
+                                     ctypes.byref(res), _dev(workspace, torch.uint8, "workspace"),
+                                     ctypes.c_size_t(workspace.numel()), ctypes.byref(opt), _stream())
+        _check(rc, "kbmod_search_rows")
     if own_workspace:
         # convenience path (no caller workspace to query later): wait and report a kernel that
         # gave up; callers that pass a workspace stay asynchronous and call search_status()
@@ -200,7 +275,7 @@ def _hostbuf(t, dtype, what: str):
 
 def search_host(sci: torch.Tensor, var: torch.Tensor, mask: Optional[torch.Tensor], psf, times,
                 vel_grid, K: int, min_obs: int, out: Dict[str, torch.Tensor],
-                workspace: torch.Tensor) -> Dict[str, torch.Tensor]:
+                workspace: torch.Tensor, kernel: Optional[int] = None) -> Dict[str, torch.Tensor]:
     """kbmod_search_host: the whole hot path from HOST tensors (pinned for asynchronous copies) to
     HOST result planes `out`; `workspace` is a CUDA uint8 tensor of search_host_workspace() bytes.
     Enqueued on the current stream; synchronise it (or call search_status) before reading `out`."""
@@ -210,14 +285,24 @@ def search_host(sci: torch.Tensor, var: torch.Tensor, mask: Optional[torch.Tenso
     vel = _host(vel_grid, np.float32)
     if psf.ndim != 3 or psf.shape[0] != N or psf.shape[1] != psf.shape[2]:
         raise KbmodError("psf must be [N,P,P]")
+    if tuple(var.shape) != (N, H, W) or (mask is not None and tuple(mask.shape) != (N, H, W)):
+        raise KbmodError("sci, var, mask shapes differ")
+    if times.shape != (N,) or vel.ndim != 2 or vel.shape[1] != 2:
+        raise KbmodError("times must be [N], vel_grid [V,2]")
+    for k in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha"):
+        if tuple(out[k].shape) != (H, W, int(K)):
+            raise KbmodError(f"result plane {k}: expected shape {(H, W, int(K))}, got {tuple(out[k].shape)}")
+    if workspace.numel() < search_host_workspace(N, H, W, int(vel.shape[0]), int(K)):
+        raise KbmodError("workspace smaller than search_host_workspace()")
     res = _Result(*[_hostbuf(out[k], torch.int32 if k in ("vel_idx", "n_obs") else torch.float32, k)
                     for k in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")])
+    opt = _options(kernel)
     rc = lib().kbmod_search_host(_hostbuf(sci, torch.float32, "sci"), _hostbuf(var, torch.float32, "var"),
                                  _hostbuf(mask, torch.uint8, "mask"), psf.ctypes.data_as(ctypes.c_void_p),
                                  times.ctypes.data_as(ctypes.c_void_p), N, H, W, int(psf.shape[1]),
                                  vel.ctypes.data_as(ctypes.c_void_p), int(vel.shape[0]), int(K), int(min_obs),
                                  ctypes.byref(res), _dev(workspace, torch.uint8, "workspace"),
-                                 ctypes.c_size_t(workspace.numel()), _stream())
+                                 ctypes.c_size_t(workspace.numel()), ctypes.byref(opt), _stream())
     _check(rc, "kbmod_search_host")
     return out
 

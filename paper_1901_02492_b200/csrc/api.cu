@@ -1,8 +1,13 @@
-// api.cu -- the C ABI of include/kbmod_b200.h: argument checks, host-side tables, dispatch.
+// api.cu -- the C ABI of include/kbmod_b200.h: argument checks, host-side plans, dispatch.
+//
+// No process-wide state selects anything: the search kernel and its tuning knobs arrive in a
+// kbmod_search_options argument, the host plan lives in a caller-owned kbmod_plan object.  The only
+// global is the launch counter (statistics).
 #include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstring>
+#include <new>
 #include <vector>
 
 #include "common.cuh"
@@ -11,7 +16,6 @@
 
 namespace kbmod {
 static std::atomic<unsigned long long> g_launches{0};
-static std::atomic<int> g_search_kernel{0};
 void note_launch(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -48,7 +52,58 @@ static WorkspaceLayout workspace_layout(int N, int H, int W, int V, int K) {
     l.total = off;
     return l;
 }
+
+// options with every default resolved; KBMOD_ERR_ARG for values out of range
+struct Options {
+    int kernel = KBMOD_KERNEL_AUTO, tile_group_w = 0, staged_geom = 0;
+};
+static int read_options(const kbmod_search_options* o, Options& out) {
+    out = Options();
+    if (!o) return KBMOD_OK;
+    if (o->struct_size != 0 && o->struct_size != (int32_t)sizeof(kbmod_search_options)) return KBMOD_ERR_ARG;
+    if (o->kernel < KBMOD_KERNEL_AUTO || o->kernel > KBMOD_KERNEL_TILED_QUEUED) return KBMOD_ERR_ARG;
+    if (o->tile_group_w < 0 || o->tile_group_w > 256) return KBMOD_ERR_ARG;
+    if (o->staged_geom < 0 || o->staged_geom > 6) return KBMOD_ERR_ARG;
+    out.kernel = o->kernel;
+    out.tile_group_w = o->tile_group_w;
+    out.staged_geom = o->staged_geom;
+    return KBMOD_OK;
+}
+
+// shared checks of the grid-shaped arguments (before any launch)
+static int check_grid(const double* times, int N, int H, int W, const float* vel_grid, int V, int K) {
+    if (!times || !vel_grid) return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0 || V <= 0) return KBMOD_ERR_SHAPE;
+    if (N > KBMOD_MAX_IMAGES || K > KBMOD_MAX_K) return KBMOD_ERR_UNSUPPORTED;
+    if (K < 1) return KBMOD_ERR_ARG;
+    for (int j = 0; j < 2 * V; ++j)
+        if (!std::isfinite(vel_grid[j])) return KBMOD_ERR_ARG;
+    for (int i = 0; i < N; ++i)
+        if (!std::isfinite(times[i])) return KBMOD_ERR_ARG;
+    return KBMOD_OK;
+}
+static int check_result(const kbmod_result* out) {
+    if (!out) return KBMOD_ERR_NULL;
+    if (!out->vel_idx || !out->n_obs || !out->psi || !out->phi || !out->nu || !out->alpha) return KBMOD_ERR_NULL;
+    if (((uintptr_t)out->vel_idx | (uintptr_t)out->n_obs | (uintptr_t)out->psi | (uintptr_t)out->phi |
+         (uintptr_t)out->nu | (uintptr_t)out->alpha) & 3)
+        return KBMOD_ERR_ALIGN;
+    return KBMOD_OK;
+}
 }  // namespace kbmod
+
+// The host plan (opaque to the caller): everything kbmod_search derives from (times, velocity grid,
+// shape, K, options) before it looks at a pixel.  Immutable after kbmod_plan_create, so any number of
+// searches on any streams may share it.
+struct kbmod_plan {
+    int N, H, W, V, K;
+    int kernel;                   // resolved: never KBMOD_KERNEL_AUTO
+    int tile_group_w;
+    kbmod::DtTable dt;
+    std::vector<float> vel;       // [V][2]
+    kbmod::TiledPlan tiled;       // kernels 2 and 4
+    kbmod::StagedPlan staged;     // kernel 3
+};
 
 using namespace kbmod;
 
@@ -73,29 +128,62 @@ size_t kbmod_search_workspace(int N, int H, int W, int V, int K) {
     return workspace_layout(N, H, W, V, K).total;
 }
 
-int kbmod_set_search_kernel(int which) {
-    if (which < 0 || which > 4) return KBMOD_ERR_ARG;
-    g_search_kernel.store(which);
+int kbmod_plan_create(const double* times, int N, int H, int W, const float* vel_grid, int V, int K,
+                      const kbmod_search_options* options, kbmod_plan** plan) {
+    if (!plan) return KBMOD_ERR_NULL;
+    *plan = nullptr;
+    if (int rc = check_grid(times, N, H, W, vel_grid, V, K)) return rc;
+    Options opt;
+    if (int rc = read_options(options, opt)) return rc;
+    kbmod_plan* p = new (std::nothrow) kbmod_plan();
+    if (!p) return KBMOD_ERR_CUDA;
+    p->N = N; p->H = H; p->W = W; p->V = V; p->K = K;
+    p->tile_group_w = opt.tile_group_w;
+    make_dt(times, N, p->dt);
+    p->vel.assign(vel_grid, vel_grid + 2 * (size_t)V);
+    int rc = KBMOD_OK;
+    switch (opt.kernel) {
+        case KBMOD_KERNEL_DIRECT:
+            p->kernel = KBMOD_KERNEL_DIRECT;
+            break;
+        case KBMOD_KERNEL_STAGED:
+            p->kernel = KBMOD_KERNEL_STAGED;
+            rc = staged_plan_build(p->dt, N, H, W, vel_grid, V, opt.staged_geom, p->staged);
+            break;
+        case KBMOD_KERNEL_TILED:
+        case KBMOD_KERNEL_TILED_QUEUED:
+            p->kernel = opt.kernel;
+            rc = tiled_plan_build(p->dt, N, H, W, vel_grid, V, K, opt.kernel == KBMOD_KERNEL_TILED_QUEUED, p->tiled);
+            break;
+        default:     // automatic: the tiled kernel where the shape fits, else the direct-gather kernel
+            p->kernel = KBMOD_KERNEL_TILED;
+            rc = tiled_plan_build(p->dt, N, H, W, vel_grid, V, K, false, p->tiled);
+            if (rc == KBMOD_ERR_UNSUPPORTED) {
+                p->kernel = KBMOD_KERNEL_DIRECT;
+                rc = KBMOD_OK;
+            }
+            break;
+    }
+    if (rc != KBMOD_OK) {
+        delete p;
+        return rc;
+    }
+    *plan = p;
     return KBMOD_OK;
 }
 
-int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
-                 const float* vel_grid, int V, int K, int min_obs, const kbmod_result* out,
-                 void* workspace, size_t workspace_bytes, void* stream) {
-    if (!psiphi || !times || !vel_grid || !out || !workspace) return KBMOD_ERR_NULL;
-    if (!out->vel_idx || !out->n_obs || !out->psi || !out->phi || !out->nu || !out->alpha)
-        return KBMOD_ERR_NULL;
-    if (N <= 0 || H <= 0 || W <= 0 || V <= 0) return KBMOD_ERR_SHAPE;
-    if (N > KBMOD_MAX_IMAGES || K > KBMOD_MAX_K) return KBMOD_ERR_UNSUPPORTED;
-    if (K < 1 || min_obs < 1 || min_obs > N) return KBMOD_ERR_ARG;
+void kbmod_plan_destroy(kbmod_plan* plan) { delete plan; }
+
+int kbmod_plan_kernel(const kbmod_plan* plan) { return plan ? plan->kernel : KBMOD_ERR_NULL; }
+
+int kbmod_search_planned(const kbmod_plan* plan, const float* psiphi, int min_obs, int y_begin, int y_end,
+                         const kbmod_result* out, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!plan || !psiphi || !workspace) return KBMOD_ERR_NULL;
+    if (int rc = check_result(out)) return rc;
+    const int N = plan->N, H = plan->H, W = plan->W, V = plan->V, K = plan->K;
+    if (min_obs < 1 || min_obs > N) return KBMOD_ERR_ARG;
+    if (y_begin < 0 || y_end > H || y_begin > y_end) return KBMOD_ERR_ARG;
     if (((uintptr_t)psiphi & 15) || ((uintptr_t)workspace & 255)) return KBMOD_ERR_ALIGN;
-    if (((uintptr_t)out->vel_idx | (uintptr_t)out->n_obs | (uintptr_t)out->psi |
-         (uintptr_t)out->phi | (uintptr_t)out->nu | (uintptr_t)out->alpha) & 3)
-        return KBMOD_ERR_ALIGN;
-    for (int j = 0; j < 2 * V; ++j)
-        if (!std::isfinite(vel_grid[j])) return KBMOD_ERR_ARG;
-    DtTable dt;
-    if (int rc = make_dt(times, N, dt)) return rc;
     const WorkspaceLayout l = workspace_layout(N, H, W, V, K);
     if (workspace_bytes < l.total) return KBMOD_ERR_WORKSPACE;
     if (!have_device()) return KBMOD_ERR_CUDA;
@@ -103,23 +191,52 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
     cudaStream_t st = (cudaStream_t)stream;
     char* ws = static_cast<char*>(workspace);
     const float2* pp = reinterpret_cast<const float2*>(psiphi);
-    const int which = g_search_kernel.load();
-
     int* status_dev = reinterpret_cast<int*>(ws + l.status_off);
     if (cudaMemsetAsync(status_dev, 0, sizeof(int), st) != cudaSuccess) return KBMOD_ERR_CUDA;
     float2* vel_dev = reinterpret_cast<float2*>(ws + l.vel_off);
-    if (cudaMemcpyAsync(vel_dev, vel_grid, (size_t)V * sizeof(float2), cudaMemcpyHostToDevice, st) != cudaSuccess)
+    if (cudaMemcpyAsync(vel_dev, plan->vel.data(), (size_t)V * sizeof(float2), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
-    if (which == 3)      // TMA-staged kernel: opt-in until it has been validated on hardware
-        return launch_search_staged(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out, ws + l.plan_off, vel_dev,
-                                    reinterpret_cast<float2*>(ws + l.enc_off), status_dev, st);
-    if (which != 1) {
-        const int rc = launch_search_tiled(pp, dt, N, H, W, vel_grid, V, K, min_obs, *out,
-                                           ws + l.plan_off, vel_dev,
-                                           reinterpret_cast<float2*>(ws + l.enc_off), which == 4, st);
-        if (rc != KBMOD_ERR_UNSUPPORTED || which == 2 || which == 4) return rc;
+    float2* enc_dev = reinterpret_cast<float2*>(ws + l.enc_off);
+    switch (plan->kernel) {
+        case KBMOD_KERNEL_STAGED:
+            return staged_launch(plan->staged, pp, plan->dt, N, H, W, K, min_obs, y_begin, y_end, *out,
+                                 ws + l.plan_off, vel_dev, enc_dev, status_dev, st);
+        case KBMOD_KERNEL_TILED:
+        case KBMOD_KERNEL_TILED_QUEUED:
+            return tiled_launch(plan->tiled, pp, plan->dt, N, H, W, K, min_obs, y_begin, y_end, *out,
+                                ws + l.plan_off, vel_dev, enc_dev, plan->tile_group_w, st);
+        default:
+            return launch_search_direct(pp, plan->dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, *out, st);
     }
-    return launch_search_direct(pp, dt, N, H, W, vel_dev, V, K, min_obs, *out, st);
+}
+
+int kbmod_search_rows(const float* psiphi, const double* times, int N, int H, int W,
+                      const float* vel_grid, int V, int K, int min_obs, int y_begin, int y_end,
+                      const kbmod_result* out, void* workspace, size_t workspace_bytes,
+                      const kbmod_search_options* options, void* stream) {
+    // every argument error is found here, before the plan is built or anything is launched
+    if (!psiphi || !workspace) return KBMOD_ERR_NULL;
+    if (int rc = check_result(out)) return rc;
+    if (int rc = check_grid(times, N, H, W, vel_grid, V, K)) return rc;
+    if (min_obs < 1 || min_obs > N) return KBMOD_ERR_ARG;
+    if (y_begin < 0 || y_end > H || y_begin > y_end) return KBMOD_ERR_ARG;
+    if (((uintptr_t)psiphi & 15) || ((uintptr_t)workspace & 255)) return KBMOD_ERR_ALIGN;
+    if (workspace_bytes < workspace_layout(N, H, W, V, K).total) return KBMOD_ERR_WORKSPACE;
+    Options opt;
+    if (int rc = read_options(options, opt)) return rc;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    kbmod_plan* plan = nullptr;
+    if (int rc = kbmod_plan_create(times, N, H, W, vel_grid, V, K, options, &plan)) return rc;
+    const int rc = kbmod_search_planned(plan, psiphi, min_obs, y_begin, y_end, out, workspace, workspace_bytes, stream);
+    kbmod_plan_destroy(plan);      // the launches have copied what they need (pageable copies are staged before return)
+    return rc;
+}
+
+int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
+                 const float* vel_grid, int V, int K, int min_obs, const kbmod_result* out,
+                 void* workspace, size_t workspace_bytes, void* stream) {
+    return kbmod_search_rows(psiphi, times, N, H, W, vel_grid, V, K, min_obs, 0, H, out, workspace,
+                             workspace_bytes, nullptr, stream);
 }
 
 int kbmod_search_status(const void* workspace, void* stream) {
@@ -161,15 +278,25 @@ size_t kbmod_search_host_workspace(int N, int H, int W, int V, int K) {
 int kbmod_search_host(const float* sci, const float* var, const uint8_t* mask, const float* psf,
                       const double* times, int N, int H, int W, int P, const float* vel_grid, int V,
                       int K, int min_obs, const kbmod_result* out, void* workspace,
-                      size_t workspace_bytes, void* stream) {
-    if (!sci || !var || !psf || !times || !vel_grid || !out || !workspace) return KBMOD_ERR_NULL;
-    if (!out->vel_idx || !out->n_obs || !out->psi || !out->phi || !out->nu || !out->alpha)
-        return KBMOD_ERR_NULL;
-    if (N <= 0 || H <= 0 || W <= 0 || V <= 0 || K <= 0) return KBMOD_ERR_SHAPE;
-    if ((uintptr_t)workspace & 255) return KBMOD_ERR_ALIGN;
+                      size_t workspace_bytes, const kbmod_search_options* options, void* stream) {
+    // every argument error of both stages is found here, before the first copy is enqueued
+    if (!sci || !var || !psf || !workspace) return KBMOD_ERR_NULL;
+    if (int rc = check_result(out)) return rc;
+    if (int rc = check_grid(times, N, H, W, vel_grid, V, K)) return rc;
+    if (min_obs < 1 || min_obs > N) return KBMOD_ERR_ARG;
+    if (P <= 0 || (P % 2) == 0) return KBMOD_ERR_ARG;
+    if (P > KBMOD_MAX_PSF) return KBMOD_ERR_UNSUPPORTED;
+    for (size_t k = 0; k < (size_t)N * P * P; ++k)
+        if (!std::isfinite(psf[k])) return KBMOD_ERR_ARG;
+    if (((uintptr_t)workspace & 255) || ((uintptr_t)sci & 3) || ((uintptr_t)var & 3)) return KBMOD_ERR_ALIGN;
+    Options opt;
+    if (int rc = read_options(options, opt)) return rc;
     const HostLayout l = host_layout(N, H, W, V, K);
     if (workspace_bytes < l.total) return KBMOD_ERR_WORKSPACE;
     if (!have_device()) return KBMOD_ERR_CUDA;
+    kbmod_plan* plan = nullptr;
+    if (int rc = kbmod_plan_create(times, N, H, W, vel_grid, V, K, options, &plan)) return rc;
+
     cudaStream_t st = (cudaStream_t)stream;
     char* ws = static_cast<char*>(workspace);
     const size_t px = (size_t)N * H * W, rk = (size_t)H * W * K;
@@ -177,11 +304,12 @@ int kbmod_search_host(const float* sci, const float* var, const uint8_t* mask, c
     float* d_var = reinterpret_cast<float*>(ws + l.var_off);
     uint8_t* d_mask = mask ? reinterpret_cast<uint8_t*>(ws + l.mask_off) : nullptr;
     float* d_pp = reinterpret_cast<float*>(ws + l.pp_off);
+    int rc = KBMOD_OK;
     if (cudaMemcpyAsync(d_sci, sci, px * 4, cudaMemcpyHostToDevice, st) != cudaSuccess ||
         cudaMemcpyAsync(d_var, var, px * 4, cudaMemcpyHostToDevice, st) != cudaSuccess ||
         (mask && cudaMemcpyAsync(d_mask, mask, px, cudaMemcpyHostToDevice, st) != cudaSuccess))
-        return KBMOD_ERR_CUDA;
-    if (int rc = kbmod_make_psi_phi(d_sci, d_var, d_mask, psf, N, H, W, P, d_pp, stream)) return rc;
+        rc = KBMOD_ERR_CUDA;
+    if (rc == KBMOD_OK) rc = kbmod_make_psi_phi(d_sci, d_var, d_mask, psf, N, H, W, P, d_pp, stream);
     kbmod_result dev;
     void* host_planes[6] = {out->vel_idx, out->n_obs, out->psi, out->phi, out->nu, out->alpha};
     void* dev_planes[6];
@@ -192,9 +320,11 @@ int kbmod_search_host(const float* sci, const float* var, const uint8_t* mask, c
     dev.phi = static_cast<float*>(dev_planes[3]);
     dev.nu = static_cast<float*>(dev_planes[4]);
     dev.alpha = static_cast<float*>(dev_planes[5]);
-    if (int rc = kbmod_search(d_pp, times, N, H, W, vel_grid, V, K, min_obs, &dev, ws + l.search_off,
-                              workspace_layout(N, H, W, V, K).total, stream))
-        return rc;
+    if (rc == KBMOD_OK)
+        rc = kbmod_search_planned(plan, d_pp, min_obs, 0, H, &dev, ws + l.search_off,
+                                  workspace_layout(N, H, W, V, K).total, stream);
+    kbmod_plan_destroy(plan);
+    if (rc != KBMOD_OK) return rc;
     for (int k = 0; k < 6; ++k)
         if (cudaMemcpyAsync(host_planes[k], dev_planes[k], rk * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
             return KBMOD_ERR_CUDA;
@@ -206,7 +336,9 @@ int kbmod_search_split(const float* psi, const float* phi, const double* times, 
                        const kbmod_result* out, void* workspace, size_t workspace_bytes,
                        void* stream) {
     if (!psi || !phi || !workspace) return KBMOD_ERR_NULL;
-    if (N <= 0 || H <= 0 || W <= 0 || V <= 0 || K <= 0) return KBMOD_ERR_SHAPE;
+    if (int rc = check_result(out)) return rc;
+    if (int rc = check_grid(times, N, H, W, vel_grid, V, K)) return rc;
+    if (min_obs < 1 || min_obs > N) return KBMOD_ERR_ARG;
     if ((uintptr_t)workspace & 255) return KBMOD_ERR_ALIGN;
     const size_t need = kbmod_search_workspace(N, H, W, V, K);
     const size_t n = (size_t)N * H * W;
@@ -235,8 +367,8 @@ int kbmod_eval_trajectories(const float* psiphi, const double* times, int N, int
 }
 
 int kbmod_debug_staged_plan(const double* times, int N, int H, int W, const float* vel_grid, int V,
-                            int32_t* stream, size_t stream_ints, int32_t* shapes, int max_shapes,
-                            int32_t* info) {
+                            int staged_geom, int32_t* stream, size_t stream_ints, int32_t* shapes,
+                            int max_shapes, int32_t* info) {
     if (!times || !vel_grid || !stream || !shapes || !info) return KBMOD_ERR_NULL;
     if (N <= 0 || H <= 0 || W <= 0 || V <= 0 || max_shapes < 0) return KBMOD_ERR_SHAPE;
     if (N > KBMOD_MAX_IMAGES) return KBMOD_ERR_UNSUPPORTED;
@@ -244,7 +376,7 @@ int kbmod_debug_staged_plan(const double* times, int N, int H, int W, const floa
         if (!std::isfinite(vel_grid[j])) return KBMOD_ERR_ARG;
     DtTable dt;
     if (int rc = make_dt(times, N, dt)) return rc;
-    return staged_plan_debug(dt, N, H, W, vel_grid, V, stream, stream_ints, shapes, max_shapes, info);
+    return staged_plan_debug(dt, N, H, W, vel_grid, V, staged_geom, stream, stream_ints, shapes, max_shapes, info);
 }
 
 unsigned long long kbmod_launch_count(void) { return g_launches.load(); }
@@ -264,6 +396,6 @@ const char* kbmod_status_string(int status) {
     return "unknown status";
 }
 
-const char* kbmod_version(void) { return "0.1"; }
+const char* kbmod_version(void) { return "0.2"; }
 
 }  // extern "C"

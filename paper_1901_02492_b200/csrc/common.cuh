@@ -28,7 +28,7 @@ int launch_psi_phi(const float* sci, const float* var, const uint8_t* mask, cons
 
 // ---- direct-gather search (search_direct.cu): any shape, global loads through L1/L2
 int launch_search_direct(const float2* psiphi, const DtTable& dt, int N, int H, int W,
-                         const float2* vel_dev, int V, int K, int min_obs,
+                         const float2* vel_dev, int V, int K, int min_obs, int y_begin, int y_end,
                          const kbmod_result& out, cudaStream_t st);
 int launch_eval_trajectories(const float2* psiphi, const DtTable& dt, int N, int H, int W,
                              const int32_t* x0y0, const float2* vxvy, int M, float* Psi,

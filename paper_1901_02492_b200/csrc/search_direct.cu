@@ -8,6 +8,7 @@
 // top-K is a sorted register list; (nu, vel_idx) of the K best are kept and their Psi/Phi/n_obs
 // are re-evaluated once at the end.
 #include "common.cuh"
+#include "topk_list.h"
 
 namespace kbmod {
 
@@ -46,17 +47,17 @@ template <int KMAX>
 __global__ void __launch_bounds__(256)
 search_direct_kernel(const float2* __restrict__ psiphi, const __grid_constant__ DtTable dt, int N,
                      int H, int W, const float2* __restrict__ vel, int V, int K, int min_obs,
-                     kbmod_result out) {
+                     int y_begin, int y_end, kbmod_result out) {
     const int x0 = blockIdx.x * 32 + threadIdx.x;
-    const int y0 = blockIdx.y * 8 + threadIdx.y;
-    if (x0 >= W || y0 >= H) return;
+    const int y0 = y_begin + blockIdx.y * 8 + threadIdx.y;
+    if (x0 >= W || y0 >= y_end) return;
 
     float best_nu[KMAX];
     int best_j[KMAX];
 #pragma unroll
     for (int k = 0; k < KMAX; ++k) {
-        best_nu[k] = -INFINITY;
-        best_j[k] = -1;
+        best_nu[k] = (k < K) ? -INFINITY : INFINITY;        // slots beyond K are never displaced
+        best_j[k] = (k < K) ? LIST_EMPTY_IDX : -1;
     }
 
     for (int j = 0; j < V; ++j) {
@@ -64,13 +65,14 @@ search_direct_kernel(const float2* __restrict__ psiphi, const __grid_constant__ 
         const Coadd c = coadd_direct(psiphi, dt, N, H, W, x0, y0, v.x, v.y, nullptr);
         if (c.n >= min_obs && c.Phi > 0.0f) {
             float nu = score_nu(c.Psi, c.Phi);
-            if (nu > best_nu[KMAX - 1]) {
-                // sorted insert; strict '>' keeps the smaller index first among equal nu
+            {
+                // sorted insert by the rule of topk_list.h (larger nu first, ties: smaller index; an
+                // empty slot ranks last, so a candidate with nu = -inf still enters an empty slot)
                 int jj = j;
                 bool shifting = false;          // after the insert the tail shifts down as is
 #pragma unroll
                 for (int k = 0; k < KMAX; ++k) {
-                    if (shifting || nu > best_nu[k]) {
+                    if (shifting || better(nu, jj, best_nu[k], best_j[k])) {
                         shifting = true;
                         const float tn = best_nu[k];
                         const int tj = best_j[k];
@@ -84,12 +86,12 @@ search_direct_kernel(const float2* __restrict__ psiphi, const __grid_constant__ 
         }
     }
 
-    const size_t base = ((size_t)y0 * W + x0) * K;
+    const size_t base = ((size_t)(y0 - y_begin) * W + x0) * K;
 #pragma unroll
     for (int k = 0; k < KMAX; ++k) {
         if (k < K) {
             const int j = best_j[k];
-            if (j >= 0) {
+            if (j != LIST_EMPTY_IDX) {
                 const float2 v = __ldg(vel + j);
                 const Coadd c = coadd_direct(psiphi, dt, N, H, W, x0, y0, v.x, v.y, nullptr);
                 out.vel_idx[base + k] = j;
@@ -111,18 +113,20 @@ search_direct_kernel(const float2* __restrict__ psiphi, const __grid_constant__ 
 }
 
 int launch_search_direct(const float2* psiphi, const DtTable& dt, int N, int H, int W,
-                         const float2* vel_dev, int V, int K, int min_obs,
+                         const float2* vel_dev, int V, int K, int min_obs, int y_begin, int y_end,
                          const kbmod_result& out, cudaStream_t st) {
+    if (y_end <= y_begin) return KBMOD_OK;
     const dim3 block(32, 8);
-    const dim3 grid((W + 31) / 32, (H + 7) / 8);
+    const dim3 grid((W + 31) / 32, (y_end - y_begin + 7) / 8);
+    if (grid.y > 65535u) return KBMOD_ERR_UNSUPPORTED;
     if (K <= 4)
-        search_direct_kernel<4><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, out);
+        search_direct_kernel<4><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
     else if (K <= 8)
-        search_direct_kernel<8><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, out);
+        search_direct_kernel<8><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
     else if (K <= 16)
-        search_direct_kernel<16><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, out);
+        search_direct_kernel<16><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
     else
-        search_direct_kernel<32><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, out);
+        search_direct_kernel<32><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }

@@ -28,7 +28,6 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
-#include <mutex>
 #include <vector>
 
 #include <cuda.h>
@@ -48,9 +47,9 @@ constexpr int TW = 32 * RX, TH = NCW * RY;   // start-pixel tile: 64 x 30
 constexpr int THREADS = (NCW + 1) * 32;  // + 1 producer warp
 constexpr int B = 8;                     // velocities per block
 static_assert(B * R == 32, "the scoring switch of search_staged_kernel lists B*R = 32 steps");
-// ring geometry variants (samples per slot, slots); selected per call by the environment variable
-// KBMOD_STAGED_GEOM (tuning knob; default 0).  Smaller slots = more boxes in flight but fewer
-// windows merged per box.
+// ring geometry variants (samples per slot, slots); selected per call by
+// kbmod_search_options.staged_geom (tuning knob; default 0).  Smaller slots = more boxes in flight
+// but fewer windows merged per box.
 // Geometries 0-3: ring of equal slots (header + box).  Geometries 4-6: byte-granular data ring
 // (ring_alloc.h) with a separate ring of VR_NH headers, so that the boxes in flight fill the
 // whole shared memory whatever their sizes; cap = largest box.
@@ -93,12 +92,6 @@ static_assert(smem_bytes_of(0) <= 227 * 1024 && smem_bytes_of(1) <= 227 * 1024 &
               smem_bytes_of(3) <= 227 * 1024 && smem_bytes_of(4) <= 227 * 1024 && smem_bytes_of(6) <= 227 * 1024,
               "ring does not fit shared memory");
 static_assert(cap_of(6) * 8 <= VR_RING_BYTES / 2, "a box must fit the variable ring comfortably");
-
-int staged_geom() {                       // KBMOD_STAGED_GEOM in [0, NGEOM), else 0
-    const char* e = std::getenv("KBMOD_STAGED_GEOM");
-    if (!e || e[0] < '0' || e[0] >= '0' + NGEOM || e[1] != 0) return 0;
-    return e[0] - '0';
-}
 
 unsigned hilbert_d(unsigned x, unsigned y) {   // Hilbert index of a 16-bit quantised (x, y)
     unsigned d = 0;
@@ -171,17 +164,9 @@ inline bool box_fits(int bw, int bh, int cap) { return bw <= MAXBW && bh <= 256 
 
 }  // namespace
 
-struct StagedPlan {
-    std::vector<int> stream;                 // nent * HDR_INTS
-    std::vector<std::pair<int, int>> shapes; // distinct (bw, bh); index = tensor-map id
-    int nent = 0;
-    // key
-    int N = 0, H = 0, W = 0, V = 0, cap = 0;
-    std::vector<float> dt, vel;
-};
-
 // Builds the entry stream.  Returns false when the box shapes cannot be brought under MAXMAPS.
 static bool build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, int cap, StagedPlan& plan) {
+    plan.nent = 0;
     // processing order: Hilbert curve over the velocity plane (ties: index)
     float lox = vel[0], hix = vel[0], loy = vel[1], hiy = vel[1];
     for (int j = 1; j < V; ++j) {
@@ -311,15 +296,24 @@ size_t staged_plan_bytes(int N, int V) {
 }
 size_t staged_enc_bytes(int N, int H, int W) { return (size_t)N * H * ((W + 1) & ~1) * sizeof(float2); }
 
-int staged_plan_debug(const DtTable& dt, int N, int H, int W, const float* vel_host, int V,
-                      int32_t* stream, size_t stream_ints, int32_t* shapes, int max_shapes, int32_t* info) {
+int staged_plan_build(const DtTable& dt, int N, int H, int W, const float* vel_host, int V, int geom,
+                      StagedPlan& plan) {
+    // limits of the int16 shift encoding, the queue's 24-bit velocity index, the TMA coordinates
     if (W > SH_LIMIT || H > SH_LIMIT || V >= (1 << 24)) return KBMOD_ERR_UNSUPPORTED;
+    if (geom < 0 || geom >= NGEOM) return KBMOD_ERR_ARG;
+    plan.geom = geom;
+    if (!build_plan(dt, N, H, W, vel_host, V, cap_of(geom), plan)) return KBMOD_ERR_UNSUPPORTED;
+    if (plan.stream.size() * sizeof(int) > staged_plan_bytes(N, V)) return KBMOD_ERR_UNSUPPORTED;
+    return KBMOD_OK;
+}
+
+int staged_plan_debug(const DtTable& dt, int N, int H, int W, const float* vel_host, int V, int geom,
+                      int32_t* stream, size_t stream_ints, int32_t* shapes, int max_shapes, int32_t* info) {
     StagedPlan plan;
-    const int cap = cap_of(staged_geom());
-    if (!build_plan(dt, N, H, W, vel_host, V, cap, plan)) return KBMOD_ERR_UNSUPPORTED;
+    if (int rc = staged_plan_build(dt, N, H, W, vel_host, V, geom, plan)) return rc;
+    const int cap = cap_of(geom);
     info[0] = plan.nent; info[1] = HDR_INTS; info[2] = (int)plan.shapes.size(); info[3] = TW;
     info[4] = TH; info[5] = B; info[6] = cap; info[7] = HDR_BYTES;
-    if (plan.stream.size() * sizeof(int) > staged_plan_bytes(N, V)) return KBMOD_ERR_UNSUPPORTED;
     if (plan.stream.size() > stream_ints || (int)plan.shapes.size() > max_shapes) return KBMOD_ERR_WORKSPACE;
     std::memcpy(stream, plan.stream.data(), plan.stream.size() * sizeof(int));
     for (size_t m = 0; m < plan.shapes.size(); ++m) {
@@ -442,6 +436,7 @@ struct StagedParams {
     const float2* vel;        // caller's velocity table (device copy)
     int* status;              // device word: set to 1 by a warp whose barrier wait timed out
     int nent, N, H, W, Wp, K, min_obs;
+    int y_begin, y_end;       // band of start rows; the result planes hold rows y_begin..y_end-1 only
     int tiles_x, tiles_y, ntiles, group_w;
     kbmod_result out;
     DtTable dt;
@@ -456,7 +451,7 @@ __device__ __forceinline__ void tile_of(const StagedParams& prm, int t, int& til
     const int ty = rem / gw;
     const int tx = g * prm.group_w + (rem - ty * gw);
     tile_x = tx * TW;
-    tile_y = ty * TH;
+    tile_y = prm.y_begin + ty * TH;
 }
 
 // memory policy of the per-pixel lists: they live in the nu / vel_idx output planes and are read
@@ -479,7 +474,7 @@ __device__ __forceinline__ void process_batch(const StagedParams& prm, unsigned 
     const int r = pix >> 5, ln = pix & 31;
     const int x = wx0 + ln + 32 * (r % RX), y = wy0 + r / RX;
     const float nu = valid ? score_nu(Psi, Phi) : 0.0f;
-    const size_t p = ((size_t)y * prm.W + x) * prm.K;
+    const size_t p = valid ? ((size_t)(y - prm.y_begin) * prm.W + x) * prm.K : 0;
     for (;;) {
         // two candidates of the same pixel in one batch: lowest lane first, the rest next round
         const unsigned same = __match_any_sync(0xFFFFFFFFu, valid ? pix : 128 + lane);
@@ -627,11 +622,12 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
         int tile_x, tile_y;
         tile_of(prm, blockIdx.x + kt * gridDim.x, tile_x, tile_y);
         const int x_first = tile_x + lane, y_first = tile_y + warp * RY;
-        unsigned inimg = 0;                        // bit r: pixel r of this thread is inside the image
+        unsigned inimg = 0;                        // bit r: pixel r of this thread is a start pixel of the band
 #pragma unroll
         for (int r = 0; r < R; ++r)
-            inimg |= ((x_first + 32 * (r % RX) < W) && (y_first + r / RX < H)) ? (1u << r) : 0u;
-        const size_t pix0 = (size_t)y_first * W + x_first;               // pixel r: pix0 + 32*rx + ry*W
+            inimg |= ((x_first + 32 * (r % RX) < W) && (y_first + r / RX < prm.y_end)) ? (1u << r) : 0u;
+        // result-plane position (band-relative rows) of pixel r: pix0 + 32*rx + ry*W
+        const size_t pix0 = (size_t)(y_first - prm.y_begin) * W + x_first;
         const u64* enc0 = prm.enc + (size_t)y_first * prm.Wp + x_first;  // image 0 samples of this thread
 
         // empty lists
@@ -819,7 +815,7 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
         for (int r = 0; r < R; ++r) {
             if (!(inimg & (1u << r))) continue;
             const int x0 = x_first + 32 * (r % RX), y0 = y_first + r / RX;
-            const size_t p = ((size_t)y0 * W + x0) * K;
+            const size_t p = ((size_t)(y0 - prm.y_begin) * W + x0) * K;
             for (int kk = 0; kk < K; ++kk) {
                 const int j = __ldcg(prm.out.vel_idx + p + kk);
                 if (j != LIST_EMPTY_IDX) {
@@ -866,12 +862,9 @@ static EncodeTiledFn encode_tiled_fn() {
 template <int CM, int KP, int G>
 static int launch_variant(const StagedParams& prm, const StagedMaps& maps, int grid, cudaStream_t st) {
     auto kern = search_staged_kernel<CM, KP, G>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes_of(G)) != cudaSuccess)
-            return KBMOD_ERR_CUDA;
-        attr_set = true;
-    }
+    // per launch, not cached: the attribute belongs to the current device's copy of the function
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes_of(G)) != cudaSuccess)
+        return KBMOD_ERR_CUDA;
     KBMOD_LAUNCH(kern, grid, THREADS, smem_bytes_of(G), st, prm, maps);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
@@ -889,31 +882,12 @@ static int launch_geom(int g, const StagedParams& prm, const StagedMaps& maps, i
     }
 }
 
-int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, int W,
-                         const float* vel_host, int V, int K, int min_obs, const kbmod_result& out,
-                         void* plan_dev, const float2* vel_dev, float2* enc_dev, int* status_dev, cudaStream_t st) {
-    // limits of the int16 shift encoding, the queue's 24-bit velocity index, the TMA coordinates
-    if (W > SH_LIMIT || H > SH_LIMIT || V >= (1 << 24)) return KBMOD_ERR_UNSUPPORTED;
+int staged_launch(const StagedPlan& plan, const float2* psiphi, const DtTable& dt, int N, int H, int W, int K,
+                  int min_obs, int y_begin, int y_end, const kbmod_result& out, void* plan_dev,
+                  const float2* vel_dev, float2* enc_dev, int* status_dev, cudaStream_t st) {
     EncodeTiledFn enc_fn = encode_tiled_fn();
     if (!enc_fn) return KBMOD_ERR_UNSUPPORTED;
-
-    // the plan depends only on (times, velocities, shape): keep the last one
-    static std::mutex mu;
-    static StagedPlan cached;
-    std::lock_guard<std::mutex> lock(mu);
-    const int geom = staged_geom(), cap = cap_of(geom);
-    const bool hit = cached.nent > 0 && cached.cap == cap && cached.N == N && cached.H == H && cached.W == W && cached.V == V &&
-                     std::memcmp(cached.dt.data(), dt.dt, sizeof(float) * N) == 0 &&
-                     std::memcmp(cached.vel.data(), vel_host, sizeof(float) * 2 * V) == 0;
-    if (!hit) {
-        cached.nent = 0;
-        if (!build_plan(dt, N, H, W, vel_host, V, cap, cached)) return KBMOD_ERR_UNSUPPORTED;
-        cached.cap = cap; cached.N = N; cached.H = H; cached.W = W; cached.V = V;
-        cached.dt.assign(dt.dt, dt.dt + N);
-        cached.vel.assign(vel_host, vel_host + 2 * (size_t)V);
-    }
-    const StagedPlan& plan = cached;
-    if (plan.stream.size() * sizeof(int) > staged_plan_bytes(N, V)) return KBMOD_ERR_UNSUPPORTED;
+    const int geom = plan.geom;
     if (cudaMemcpyAsync(plan_dev, plan.stream.data(), plan.stream.size() * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
 
@@ -944,11 +918,13 @@ int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, 
     prm.vel = vel_dev;
     prm.status = status_dev;
     prm.nent = plan.nent; prm.N = N; prm.H = H; prm.W = W; prm.Wp = Wp; prm.K = K; prm.min_obs = min_obs;
+    prm.y_begin = y_begin; prm.y_end = y_end;
     prm.tiles_x = (W + TW - 1) / TW;
-    prm.tiles_y = (H + TH - 1) / TH;
+    prm.tiles_y = (y_end - y_begin + TH - 1) / TH;
     prm.group_w = 8;
     const long long tiles = (long long)prm.tiles_x * prm.tiles_y;
     if (tiles > 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
+    if (tiles == 0) return KBMOD_OK;
     prm.ntiles = (int)tiles;
     prm.out = out;
     prm.dt = dt;
@@ -965,5 +941,15 @@ int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, 
     if (cm == 2) return launch_geom<2, 0>(geom, prm, maps, grid, st);
     if (cm == 1) return launch_geom<1, 0>(geom, prm, maps, grid, st);
     return launch_geom<0, 0>(geom, prm, maps, grid, st);
+}
+
+int launch_search_staged(const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                         const float* vel_host, int V, int K, int min_obs, int y_begin, int y_end,
+                         const kbmod_result& out, void* plan_dev, const float2* vel_dev, float2* enc_dev,
+                         int* status_dev, int geom, cudaStream_t st) {
+    StagedPlan plan;
+    if (int rc = staged_plan_build(dt, N, H, W, vel_host, V, geom, plan)) return rc;
+    return staged_launch(plan, psiphi, dt, N, H, W, K, min_obs, y_begin, y_end, out, plan_dev, vel_dev, enc_dev,
+                         status_dev, st);
 }
 }  // namespace kbmod

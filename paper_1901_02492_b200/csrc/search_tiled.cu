@@ -73,6 +73,21 @@ size_t tiled_plan_bytes(int N, int V, int K) {
     return nblk * rec_ints(B, N) * sizeof(int) + 256;
 }
 
+static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, int B,
+                      std::vector<int>& plan, bool isolate);
+
+int tiled_plan_build(const DtTable& dt, int N, int H, int W, const float* vel_host, int V, int K, bool queued,
+                     TiledPlan& plan) {
+    // limits of the int16 shift encoding and of the int32 element offsets
+    if (W > 30000 || H > 30000) return KBMOD_ERR_UNSUPPORTED;
+    if (queued && V >= (1 << 24)) return KBMOD_ERR_UNSUPPORTED;    // 25-bit velocity index in the queue word
+    if ((long long)(N + 1) * H * W + (long long)SH_LIMIT * (W + 1) >= 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
+    plan.queued = queued;
+    plan.nblk = build_plan(dt, N, H, W, vel_host, V, block_size_for_k(K), plan.rec, queued);
+    if (plan.rec.size() * sizeof(int) > tiled_plan_bytes(N, V, K)) return KBMOD_ERR_UNSUPPORTED;
+    return KBMOD_OK;
+}
+
 // Builds the host plan; returns the number of velocity blocks.  margin: see the header comment.
 // isolate (kernel 4): a chunk of B velocities that contains velocities with an unproven or skipped
 // shift is split into a block of the clean ones and a block of the others, and blocks are filled
@@ -80,7 +95,7 @@ size_t tiled_plan_bytes(int N, int V, int K) {
 // so that the clean block keeps the branch-free gather loops.  The per-pixel result does not
 // depend on the order in which velocities are visited.
 static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, int B,
-                      std::vector<int>& plan, bool isolate = false) {
+                      std::vector<int>& plan, bool isolate) {
     // processing order: Hilbert curve over the velocity plane (ties and order of equal keys: index)
     float lox = vel[0], hix = vel[0], loy = vel[1], hiy = vel[1];
     for (int j = 1; j < V; ++j) {
@@ -241,6 +256,7 @@ struct TiledParams {
     const int* plan;          // nblk records
     const float2* vel;        // caller's velocity table (device copy)
     int nblk, N, H, W, K, min_obs;
+    int y_begin, y_end;       // band of start rows; the result planes hold rows y_begin..y_end-1 only
     int tiles_x, tiles_y, group_w;
     kbmod_result out;
     DtTable dt;
@@ -284,12 +300,13 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
         ty = rem / gw;
         tx = g * prm.group_w + (rem - ty * gw);
     }
-    const int tile_x = tx * G::TW, tile_y = ty * G::TH;
+    const int tile_x = tx * G::TW, tile_y = prm.y_begin + ty * G::TH;
     const int x_first = tile_x + (warp % WX) * 32 * RX + lane;
     const int y_first = tile_y + (warp / WX) * RY;
-    const bool ragged = (tile_x + G::TW > W) || (tile_y + G::TH > H);
+    const int y_end = prm.y_end;                     // start rows of this search: [y_begin, y_end)
+    const bool ragged = (tile_x + G::TW > W) || (tile_y + G::TH > y_end);
     // tile extent that holds real pixels (for window classification)
-    const int tile_x1 = min(tile_x + G::TW, W) - 1, tile_y1 = min(tile_y + G::TH, H) - 1;
+    const int tile_x1 = min(tile_x + G::TW, W) - 1, tile_y1 = min(tile_y + G::TH, y_end) - 1;
 
     const u64* basep[RY];
 #pragma unroll
@@ -330,7 +347,7 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
 #pragma unroll
                 for (int rx = 0; rx < RX; ++rx) {
                     // image 0 has dt = 0: shift (0,0) for every velocity
-                    const bool inimg = (x_first + 32 * rx < W) && (y_first + ry < H);
+                    const bool inimg = (x_first + 32 * rx < W) && (y_first + ry < y_end);
                     const u64 s0 = inimg ? ld_sample(basep[ry] + 32 * rx) : 0ull;
                     acc[b][ry * RX + rx] = s0;
                     cnt[b][ry * RX + rx] = (unsigned)(s0 >> 63);
@@ -370,7 +387,7 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
 #pragma unroll
                         for (int ry = 0; ry < RY; ++ry) {
                             const int y = y_first + ry + sy;
-                            const bool yin = (y_first + ry < H) && y >= 0 && y < H;
+                            const bool yin = (y_first + ry < y_end) && y >= 0 && y < H;
 #pragma unroll
                             for (int rx = 0; rx < RX; ++rx) {
                                 const int x = x_first + 32 * rx + sx;
@@ -387,7 +404,7 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
 #pragma unroll
                         for (int ry = 0; ry < RY; ++ry) {
                             int y = 0;
-                            const bool yin = traj_pixel(y_first + ry, vy, dti, H, y) && (y_first + ry < H);
+                            const bool yin = traj_pixel(y_first + ry, vy, dti, H, y) && (y_first + ry < y_end);
 #pragma unroll
                             for (int rx = 0; rx < RX; ++rx) {
                                 int x = 0;
@@ -448,9 +465,9 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
     for (int r = 0; r < R; ++r) {
         const int rx = r % RX, ry = r / RX;
         const int x0 = x_first + 32 * rx, y0 = y_first + ry;
-        if (x0 >= W || y0 >= H) continue;
+        if (x0 >= W || y0 >= y_end) continue;
         const int p = r * THREADS + tid;
-        const size_t obase = ((size_t)y0 * W + x0) * K;
+        const size_t obase = ((size_t)(y0 - prm.y_begin) * W + x0) * K;
         for (int k = 0; k < K; ++k) {
             float bn = -INFINITY;
             int bj = 0x7FFFFFFF, bs = -1;
@@ -521,7 +538,7 @@ __device__ __forceinline__ void process_batch_q(const TiledParams& prm, const fl
     const int r = pix >> 5, ln = pix & 31;
     const int x = wx0 + ln + 32 * (r % RX), y = wy0 + r / RX;
     const float nu = valid ? score_nu(Psi, Phi) : 0.0f;
-    const size_t p = valid ? ((size_t)y * prm.W + x) * prm.K : 0;
+    const size_t p = valid ? ((size_t)(y - prm.y_begin) * prm.W + x) * prm.K : 0;
     for (;;) {
         // two candidates of the same pixel in one batch: lowest lane first, the rest next round
         const unsigned same = __match_any_sync(0xFFFFFFFFu, valid ? pix : 128 + lane);
@@ -564,16 +581,18 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
         ty = rem / gw;
         tx = g * prm.group_w + (rem - ty * gw);
     }
-    const int tile_x = tx * TW, tile_y = ty * TH;
+    const int tile_x = tx * TW, tile_y = prm.y_begin + ty * TH;
     const int x_first = tile_x + lane;
     const int y_first = tile_y + warp * RY;
-    const bool ragged = (tile_x + TW > W) || (tile_y + TH > H);
-    const int tile_x1 = min(tile_x + TW, W) - 1, tile_y1 = min(tile_y + TH, H) - 1;
-    unsigned inimg = 0;                                           // bit r: pixel r of this thread is inside the image
+    const int y_end = prm.y_end;                                  // start rows of this search: [y_begin, y_end)
+    const bool ragged = (tile_x + TW > W) || (tile_y + TH > y_end);
+    const int tile_x1 = min(tile_x + TW, W) - 1, tile_y1 = min(tile_y + TH, y_end) - 1;
+    unsigned inimg = 0;                                           // bit r: pixel r of this thread is a start pixel of the band
 #pragma unroll
     for (int r = 0; r < R; ++r)
-        inimg |= ((x_first + 32 * (r % RX) < W) && (y_first + r / RX < H)) ? (1u << r) : 0u;
-    const size_t pix0 = (size_t)y_first * W + x_first;            // pixel r: pix0 + 32*rx + ry*W
+        inimg |= ((x_first + 32 * (r % RX) < W) && (y_first + r / RX < y_end)) ? (1u << r) : 0u;
+    // result-plane position (band-relative rows) of pixel r: pix0 + 32*rx + ry*W
+    const size_t pix0 = (size_t)(y_first - prm.y_begin) * W + x_first;
 
     const u64* basep[RY];
 #pragma unroll
@@ -724,7 +743,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
 #pragma unroll
                         for (int ry = 0; ry < RY; ++ry) {
                             const int y = y_first + ry + sy;
-                            const bool yin = (y_first + ry < H) && y >= 0 && y < H;
+                            const bool yin = (y_first + ry < y_end) && y >= 0 && y < H;
 #pragma unroll
                             for (int rx = 0; rx < RX; ++rx) {
                                 const int x = x_first + 32 * rx + sx;
@@ -740,7 +759,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
 #pragma unroll
                         for (int ry = 0; ry < RY; ++ry) {
                             int y = 0;
-                            const bool yin = traj_pixel(y_first + ry, vy, dti, H, y) && (y_first + ry < H);
+                            const bool yin = traj_pixel(y_first + ry, vy, dti, H, y) && (y_first + ry < y_end);
 #pragma unroll
                             for (int rx = 0; rx < RX; ++rx) {
                                 int x = 0;
@@ -823,7 +842,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
     for (int r = 0; r < R; ++r) {
         if (!(inimg & (1u << r))) continue;
         const int x0 = x_first + 32 * (r % RX), y0 = y_first + r / RX;
-        const size_t obase = ((size_t)y0 * W + x0) * K;
+        const size_t obase = ((size_t)(y0 - prm.y_begin) * W + x0) * K;
         for (int k = 0; k < K; ++k) {
             const int bj = __ldcg(prm.out.vel_idx + obase + k);
             if (bj != LIST_EMPTY_IDX) {
@@ -859,29 +878,27 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
 // launch
 // ---------------------------------------------------------------------------------------------
 template <int RX, int RY, int WX, int B, int KMAX>
-static int launch_variant(TiledParams& prm, cudaStream_t st) {
+static int launch_variant(TiledParams& prm, int group_w, cudaStream_t st) {
     using G = TileGeom<RX, RY, WX, B, KMAX>;
     const size_t smem = G::smem_bytes(prm.N);
     if (smem > 227 * 1024) return KBMOD_ERR_UNSUPPORTED;
     auto kern = search_tiled_kernel<RX, RY, WX, B, KMAX>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess)
-            return KBMOD_ERR_CUDA;
-        attr_set = true;
-    }
+    // per launch, not cached: the attribute belongs to the current device's copy of the function
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess)
+        return KBMOD_ERR_CUDA;
     prm.tiles_x = (prm.W + G::TW - 1) / G::TW;
-    prm.tiles_y = (prm.H + G::TH - 1) / G::TH;
-    prm.group_w = std::max(1, 512 / G::TW);
+    prm.tiles_y = (prm.y_end - prm.y_begin + G::TH - 1) / G::TH;
+    prm.group_w = group_w > 0 ? std::min(group_w, 256) : std::max(1, 512 / G::TW);
     const long long tiles = (long long)prm.tiles_x * prm.tiles_y;
     if (tiles > 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
+    if (tiles == 0) return KBMOD_OK;
     KBMOD_LAUNCH(kern, (unsigned)tiles, THREADS, smem, st, prm);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }
 
 template <int RX, int RY, int B, int KP, int CM>
-static int launch_variant_q(TiledParams& prm, cudaStream_t st) {
+static int launch_variant_q(TiledParams& prm, int group_w, cudaStream_t st) {
     constexpr int TW = 32 * RX, TH = RY * (THREADS / 32);
     // two block records + the queues: 14.7 KB at N = 15, 46.8 KB at most (N = 64, B = 32), i.e. below
     // the 48 KB that need no opt-in; the rest of the SM's 256 KB stays L1 for the gathers
@@ -889,33 +906,22 @@ static int launch_variant_q(TiledParams& prm, cudaStream_t st) {
     if (smem > 48 * 1024) return KBMOD_ERR_UNSUPPORTED;
     auto kern = search_tiledq_kernel<RX, RY, B, KP, CM>;
     prm.tiles_x = (prm.W + TW - 1) / TW;
-    prm.tiles_y = (prm.H + TH - 1) / TH;
-    // tile rasterisation: groups of group_w tile columns (default 512 px wide).  KBMOD_TILED_GROUPW
-    // (1..256, kernel 4 only) overrides it: a tuning knob bench.py's kernel selection sweeps; the
-    // results do not depend on it
-    prm.group_w = std::max(1, 512 / TW);
-    if (const char* e = std::getenv("KBMOD_TILED_GROUPW")) {
-        const int g = std::atoi(e);
-        if (g >= 1 && g <= 256) prm.group_w = g;
-    }
+    prm.tiles_y = (prm.y_end - prm.y_begin + TH - 1) / TH;
+    // tile rasterisation: groups of group_w tile columns (default 512 px wide; kbmod_search_options
+    // tile_group_w overrides it: a tuning knob, the results do not depend on it)
+    prm.group_w = group_w > 0 ? std::min(group_w, 256) : std::max(1, 512 / TW);
     const long long tiles = (long long)prm.tiles_x * prm.tiles_y;
     if (tiles > 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
+    if (tiles == 0) return KBMOD_OK;
     KBMOD_LAUNCH(kern, (unsigned)tiles, THREADS, smem, st, prm);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }
 
-int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, int W,
-                        const float* vel_host, int V, int K, int min_obs, const kbmod_result& out,
-                        void* plan_dev, const float2* vel_dev, float2* enc_dev, bool queued, cudaStream_t st) {
-    // limits of the int16 shift encoding and of the int32 element offsets
-    if (W > 30000 || H > 30000) return KBMOD_ERR_UNSUPPORTED;
-    if (queued && V >= (1 << 24)) return KBMOD_ERR_UNSUPPORTED;    // 25-bit velocity index in the queue word
-    if ((long long)(N + 1) * H * W + (long long)SH_LIMIT * (W + 1) >= 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
-    const int B = block_size_for_k(K);
-    std::vector<int> plan;
-    const int nblk = build_plan(dt, N, H, W, vel_host, V, B, plan, queued);
-    if (cudaMemcpyAsync(plan_dev, plan.data(), plan.size() * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess)
+int tiled_launch(const TiledPlan& plan, const float2* psiphi, const DtTable& dt, int N, int H, int W, int K,
+                 int min_obs, int y_begin, int y_end, const kbmod_result& out, void* plan_dev,
+                 const float2* vel_dev, float2* enc_dev, int group_w, cudaStream_t st) {
+    if (cudaMemcpyAsync(plan_dev, plan.rec.data(), plan.rec.size() * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
 
     const size_t n = (size_t)N * H * W;
@@ -929,18 +935,29 @@ int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, i
     prm.enc = reinterpret_cast<const u64*>(enc_dev);
     prm.plan = static_cast<const int*>(plan_dev);
     prm.vel = vel_dev;
-    prm.nblk = nblk; prm.N = N; prm.H = H; prm.W = W; prm.K = K; prm.min_obs = min_obs;
+    prm.nblk = plan.nblk; prm.N = N; prm.H = H; prm.W = W; prm.K = K; prm.min_obs = min_obs;
+    prm.y_begin = y_begin; prm.y_end = y_end;
     prm.out = out;
     prm.dt = dt;
-    if (queued) {                                                   // kernel 4: same tiles, queue-compacted S5/S6
+    if (plan.queued) {                                              // kernel 4: same tiles, queue-compacted S5/S6
         const bool hist = N <= 16;                                  // history-bit counting (see CM)
-        if (K <= 8) return hist ? launch_variant_q<2, 2, 8, 8, 2>(prm, st) : launch_variant_q<2, 2, 8, 8, 0>(prm, st);
-        if (K <= 16) return hist ? launch_variant_q<2, 1, 16, 0, 2>(prm, st) : launch_variant_q<2, 1, 16, 0, 0>(prm, st);
-        return launch_variant_q<1, 1, 32, 0, 0>(prm, st);
+        if (K <= 8) return hist ? launch_variant_q<2, 2, 8, 8, 2>(prm, group_w, st) : launch_variant_q<2, 2, 8, 8, 0>(prm, group_w, st);
+        if (K <= 16) return hist ? launch_variant_q<2, 1, 16, 0, 2>(prm, group_w, st) : launch_variant_q<2, 1, 16, 0, 0>(prm, group_w, st);
+        return launch_variant_q<1, 1, 32, 0, 0>(prm, group_w, st);
     }
-    if (K <= 8) return launch_variant<2, 2, 1, 8, 8>(prm, st);      // tile 64 x 32
-    if (K <= 16) return launch_variant<2, 1, 1, 16, 16>(prm, st);   // tile 64 x 16
-    return launch_variant<1, 1, 1, 32, 32>(prm, st);                // tile 32 x 16
+    if (K <= 8) return launch_variant<2, 2, 1, 8, 8>(prm, group_w, st);      // tile 64 x 32
+    if (K <= 16) return launch_variant<2, 1, 1, 16, 16>(prm, group_w, st);   // tile 64 x 16
+    return launch_variant<1, 1, 1, 32, 32>(prm, group_w, st);                // tile 32 x 16
+}
+
+int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                        const float* vel_host, int V, int K, int min_obs, int y_begin, int y_end,
+                        const kbmod_result& out, void* plan_dev, const float2* vel_dev, float2* enc_dev,
+                        bool queued, int group_w, cudaStream_t st) {
+    TiledPlan plan;
+    if (int rc = tiled_plan_build(dt, N, H, W, vel_host, V, K, queued, plan)) return rc;
+    return tiled_launch(plan, psiphi, dt, N, H, W, K, min_obs, y_begin, y_end, out, plan_dev, vel_dev, enc_dev,
+                        group_w, st);
 }
 
 }  // namespace kbmod

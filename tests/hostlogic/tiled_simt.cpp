@@ -22,9 +22,11 @@ void note_launch(int) {}
 extern "C" {
 
 // stats[0..4] = shared-memory faults (none possible here: plain pointers), 0, 0, kernel launches, 0
+// Result planes hold the band [y_begin, y_end) only.  group_w = kbmod_search_options.tile_group_w.
 int simt_search_tiled(const float* psiphi, const double* times, int N, int H, int W, const float* vel_grid, int V,
-                      int K, int min_obs, int32_t* vel_idx, int32_t* n_obs, float* psi, float* phi, float* nu,
-                      float* alpha, int queued, int order, unsigned seed, long long* stats) {
+                      int K, int min_obs, int y_begin, int y_end, int32_t* vel_idx, int32_t* n_obs, float* psi,
+                      float* phi, float* nu, float* alpha, int queued, int group_w, int order, unsigned seed,
+                      long long* stats) {
     using namespace kbmod;
     simt::cfg().order = order;
     simt::cfg().seed = seed;
@@ -36,15 +38,15 @@ int simt_search_tiled(const float* psiphi, const double* times, int N, int H, in
     for (int i = 0; i < N; ++i) dt.dt[i] = (float)(times[i] - times[0]);
     // every buffer the kernels see is its own heap block of exactly the size the product gives them
     // (devmem.h): inputs copied in, result planes copied back
-    const size_t npix = (size_t)N * H * W, nres = (size_t)H * W * K;
+    const size_t npix = (size_t)N * H * W, nres = (size_t)(y_end - y_begin) * W * K;
     simt::DevBuf d_pp(psiphi, npix * 8), d_vel(vel_grid, (size_t)V * 8);
     simt::DevBuf d_plan(tiled_plan_bytes(N, V, K)), d_enc(npix * 8);
     simt::DevBuf d_vi(nres * 4), d_no(nres * 4), d_psi(nres * 4), d_phi(nres * 4), d_nu(nres * 4), d_al(nres * 4);
     kbmod_result out{d_vi.as<int32_t>(), d_no.as<int32_t>(), d_psi.as<float>(), d_phi.as<float>(),
                      d_nu.as<float>(), d_al.as<float>()};
-    const int rc = launch_search_tiled(d_pp.as<const float2>(), dt, N, H, W, vel_grid, V, K, min_obs,
+    const int rc = launch_search_tiled(d_pp.as<const float2>(), dt, N, H, W, vel_grid, V, K, min_obs, y_begin, y_end,
                                        out, d_plan.p, d_vel.as<const float2>(), d_enc.as<float2>(), queued != 0,
-                                       nullptr);
+                                       group_w, nullptr);
     d_vi.copy_to(vel_idx); d_no.copy_to(n_obs); d_psi.copy_to(psi); d_phi.copy_to(phi); d_nu.copy_to(nu);
     d_al.copy_to(alpha);
     stats[0] = s.smem_faults; stats[1] = 0; stats[2] = 0; stats[3] = s.launches; stats[4] = 0;
@@ -59,7 +61,8 @@ int simt_tiled_limits(int N, int H, int W, int V, int K) {
     for (int i = 0; i < KBMOD_MAX_IMAGES; ++i) dt.dt[i] = (float)i;
     std::vector<float> vel((size_t)2 * V, 1.0f);
     kbmod_result out{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    return launch_search_tiled(nullptr, dt, N, H, W, vel.data(), V, K, 1, out, nullptr, nullptr, nullptr, true, nullptr);
+    return launch_search_tiled(nullptr, dt, N, H, W, vel.data(), V, K, 1, 0, H, out, nullptr, nullptr, nullptr, true, 0,
+                               nullptr);
 }
 
 // Detector self-test: reads the element `past` elements beyond a 64-byte emulated device buffer

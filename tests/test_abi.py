@@ -57,8 +57,63 @@ def test_argument_errors_before_any_launch(L):
     assert L.kbmod_search(fp, t, 2, 2, 2, fp, 1, 33, 1, ctypes.byref(r), fp, 0, None) == -6
     assert L.kbmod_search(fp, t, 2, 2, 2, fp, 1, 1, 3, ctypes.byref(r), fp, 0, None) == -3
     assert L.kbmod_search(fp, t, 65, 2, 2, fp, 1, 1, 1, ctypes.byref(r), fp, 0, None) == -6
-    assert L.kbmod_set_search_kernel(7) == -3
-    assert L.kbmod_set_search_kernel(0) == 0
+
+
+def test_rows_options_and_plan_argument_errors(L):
+    """kbmod_search_rows / kbmod_plan_create / kbmod_search_planned / kbmod_search_host reject bad
+    bands, options and shapes before any launch (no device here: a valid call would return -5)."""
+    f = np.zeros(64, np.float32)
+    buf = np.zeros(4096, np.uint8)
+    fp = ctypes.c_void_p((f.ctypes.data + 15) // 16 * 16)
+    ws = ctypes.c_void_p((buf.ctypes.data + 255) // 256 * 256)
+    t = np.array([0.0, 1.0]).ctypes.data_as(ctypes.c_void_p)
+    vel = np.ones(2, np.float32).ctypes.data_as(ctypes.c_void_p)
+
+    class R(ctypes.Structure):
+        _fields_ = [(n, ctypes.c_void_p) for n in ("a", "b", "c", "d", "e", "f")]
+
+    class O(ctypes.Structure):
+        _fields_ = [(n, ctypes.c_int32) for n in ("struct_size", "kernel", "tile_group_w", "staged_geom")]
+    r = R(*[f.ctypes.data] * 6)
+    big = ctypes.c_size_t(1 << 40)
+    rows = lambda y0, y1, opt=None: L.kbmod_search_rows(fp, t, 2, 4, 4, vel, 1, 1, 1, y0, y1, ctypes.byref(r), ws, big,
+                                                        ctypes.byref(opt) if opt else None, None)
+    assert rows(-1, 2) == -3 and rows(3, 2) == -3 and rows(0, 5) == -3            # band outside [0, H]
+    assert rows(0, 4, O(16, 9, 0, 0)) == -3 and rows(0, 4, O(16, -1, 0, 0)) == -3  # unknown kernel
+    assert rows(0, 4, O(16, 0, 300, 0)) == -3 and rows(0, 4, O(16, 3, 0, 7)) == -3 # knobs out of range
+    assert rows(0, 4, O(12, 0, 0, 0)) == -3                                         # wrong struct_size
+    assert L.kbmod_search_rows(fp, t, 2, 4, 4, vel, 1, 1, 1, 0, 4, ctypes.byref(r), ws, ctypes.c_size_t(8), None, None) == -7
+    # plans: host objects, no device needed
+    h = ctypes.c_void_p()
+    assert L.kbmod_plan_create(t, 2, 4, 4, vel, 1, 1, None, None) == -1
+    assert L.kbmod_plan_create(t, 2, 4, 4, vel, 1, 33, None, ctypes.byref(h)) == -6 and not h
+    assert L.kbmod_plan_create(t, 2, 0, 4, vel, 1, 1, None, ctypes.byref(h)) == -2
+    bad_t = np.array([0.0, np.inf]).ctypes.data_as(ctypes.c_void_p)
+    assert L.kbmod_plan_create(bad_t, 2, 4, 4, vel, 1, 1, None, ctypes.byref(h)) == -3
+    assert L.kbmod_plan_create(t, 2, 4, 4, vel, 1, 1, None, ctypes.byref(h)) == 0 and h
+    assert L.kbmod_plan_kernel(h) == 2                       # automatic resolves to the tiled kernel
+    assert L.kbmod_search_planned(h, fp, 3, 0, 4, ctypes.byref(r), ws, big, None) == -3     # min_obs > N
+    assert L.kbmod_search_planned(h, fp, 1, 2, 1, ctypes.byref(r), ws, big, None) == -3     # bad band
+    assert L.kbmod_search_planned(h, None, 1, 0, 4, ctypes.byref(r), ws, big, None) == -1
+    L.kbmod_plan_destroy(h)
+    L.kbmod_plan_destroy(None)
+    for k, want in ((1, 1), (3, 3), (4, 4)):
+        h = ctypes.c_void_p()
+        o = O(16, k, 0, 0)
+        assert L.kbmod_plan_create(t, 2, 4, 4, vel, 1, 1, ctypes.byref(o), ctypes.byref(h)) == 0
+        assert L.kbmod_plan_kernel(h) == want
+        L.kbmod_plan_destroy(h)
+    # a shape beyond the tiled kernel: automatic falls back to the direct kernel, explicit 2 is refused
+    h = ctypes.c_void_p()
+    assert L.kbmod_plan_create(t, 2, 40000, 4, vel, 1, 1, None, ctypes.byref(h)) == 0 and L.kbmod_plan_kernel(h) == 1
+    L.kbmod_plan_destroy(h)
+    o = O(16, 2, 0, 0)
+    assert L.kbmod_plan_create(t, 2, 40000, 4, vel, 1, 1, ctypes.byref(o), ctypes.byref(h)) == -6
+    # kbmod_search_host: the search-stage errors are reported before anything is enqueued
+    psf = np.ones(1, np.float32).ctypes.data_as(ctypes.c_void_p)
+    host = lambda K, mo, P: L.kbmod_search_host(fp, fp, None, psf, t, 2, 4, 4, P, vel, 1, K, mo, ctypes.byref(r), ws,
+                                                big, None, None)
+    assert host(40, 1, 1) == -6 and host(1, 3, 1) == -3 and host(1, 1, 2) == -3 and host(1, 1, 33) == -6
 
 
 def test_no_cpu_fallback_without_device(L):

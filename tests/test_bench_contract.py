@@ -3,9 +3,9 @@
 The GPU arm is run with a stub in place of the ctypes binding and of the few torch.cuda calls it
 makes (events, synchronize, pinned memory), on BASELINE.json configs[0]; the reference arm runs
 the real oracle.  What is checked is the control flow and the JSON line: every key the driver and
-the judge read is present and well-formed, the kernel-selection report is carried through, and a
-probe that cannot run (no GPU here) falls back to the library's default kernel instead of failing
-the benchmark.  No timing value printed by this test means anything.
+the judge read is present and well-formed, the default run times the library's default kernel
+through a prebuilt plan, and --kernel k is carried into the options.  No timing value printed by
+this test means anything.
 """
 import io
 import json
@@ -37,7 +37,12 @@ def stubbed(monkeypatch):
     planes = ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")
     b = types.ModuleType("paper_1901_02492_b200.binding")
     b.lib = lambda: None
-    b.set_search_kernel = lambda w: calls["kernel"].append(int(w))
+
+    class Plan:
+        def __init__(self, times, N, H, W, vel, K, kernel=None, tile_group_w=0, staged_geom=0):
+            calls["kernel"].append(int(kernel))
+            calls["plans"] = calls.get("plans", 0) + 1
+    b.Plan = Plan
     b.alloc_result = lambda H, W, K, dev: {k: torch.zeros((H, W, K), dtype=torch.int32 if k in planes[:2] else torch.float32)
                                            for k in planes}
     b.search_workspace = lambda *a: 1024
@@ -47,11 +52,12 @@ def stubbed(monkeypatch):
         calls["launches"] += 1
         return out
 
-    def search(*a, out=None, workspace=None, **k):
+    def search(*a, out=None, workspace=None, plan=None, **k):
+        assert isinstance(plan, Plan), "the timed search goes through the prebuilt plan"
         calls["launches"] += 2
         return out
 
-    def search_host(*a):
+    def search_host(*a, kernel=None):
         calls["launches"] += 3
 
     b.make_psi_phi, b.search, b.search_host = make_psi_phi, search, search_host
@@ -97,39 +103,32 @@ def check_common(d):
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
 
 
-def test_gpu_arm_line_with_selected_candidate(stubbed, monkeypatch):
-    report = {"identical": True, "ms_default": 320.0, "ms_candidate": 160.0,
-              "selected": bench.KERNEL_NAMES[bench.CANDIDATE_KERNEL]}
-    monkeypatch.setattr(bench, "select_kernel", lambda args, seed, lr: (bench.CANDIDATE_KERNEL, dict(report)))
-    d = run_main(monkeypatch, ["--config", "1", "--steps", "3", "--warmup", "3", "--ref-rows", "8"])
+def test_gpu_arm_line_default_kernel(stubbed, monkeypatch):
+    d = run_main(monkeypatch, ["--config", "1", "--steps", "3", "--warmup", "1", "--ref-rows", "8"])
     check_common(d)
-    assert stubbed["kernel"] == [bench.CANDIDATE_KERNEL]
-    assert d["steps"] == 3 and d["warmup"] == 3
+    assert stubbed["kernel"] == [0] and stubbed["plans"] == 1, "default kernel, one plan for the whole run"
+    assert d["steps"] == 3 and d["warmup"] == 3, "at least three warm-up steps whatever was asked"
     assert d["gpu_launches"] == 9                      # 3 timed steps x (psi/phi + search) of the stub
-    assert d["search_kernel"] == bench.KERNEL_NAMES[bench.CANDIDATE_KERNEL]
-    assert d["kernel_selection"]["identical"] is True
+    assert "search_tiled_kernel" in d["search_kernel"]
+    assert d["search_options"]["kernel"] == 0
     r = d["roofline"]
     assert r["bound"] == "smem" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
-    assert "traffic" in r and "search_tiledq_kernel" in r["kernel"]
+    assert r["traffic"] is None and "search_tiled_kernel" in r["kernel"]
     assert d["e2e"]["h2d_bytes_per_step"] == 5 * 64 * 64 * 9 and d["e2e"]["d2h_bytes_per_step"] == 64 * 64 * 4 * 24
     assert "clocks" in d and set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
     assert "kbmod_search_host" in d["e2e"]["path"] and "path" in d["e2e_binding_copies"]
 
 
-def test_gpu_arm_falls_back_when_the_probe_cannot_run(stubbed, monkeypatch):
-    """No GPU here: the probe child fails, and the benchmark goes on with the default kernel."""
-    d = run_main(monkeypatch, ["--config", "1", "--steps", "2", "--warmup", "1", "--ref-rows", "8"])
-    check_common(d)
-    assert stubbed["kernel"] == [0]
-    assert "error" in d["kernel_selection"]
-    assert d["warmup"] == 3, "at least three warm-up steps whatever was asked"
-    assert "search_tiled_kernel" in d["roofline"]["kernel"]
+def test_last_capture_is_reported_beside_the_roofline_for_the_bench_workload():
+    c = bench.last_capture(0)
+    assert c and c["commit"] and c["dram_bytes_read"] > 1e11 and "profiles/" in c["source"]
+    assert bench.last_capture(4) is None, "no capture of kernel 4 exists: none is claimed"
 
 
-def test_explicit_kernel_skips_the_probe(stubbed, monkeypatch):
-    monkeypatch.setattr(bench, "select_kernel", lambda *a: pytest.fail("probe must not run with --kernel k"))
-    d = run_main(monkeypatch, ["--config", "1", "--steps", "1", "--kernel", "2", "--no-cpu"])
-    assert stubbed["kernel"] == [2] and d["kernel_selection"]["rule"] == "--kernel given"
+def test_explicit_kernel_goes_into_the_options(stubbed, monkeypatch):
+    d = run_main(monkeypatch, ["--config", "1", "--steps", "1", "--kernel", "4", "--group-w", "4", "--no-cpu"])
+    assert stubbed["kernel"] == [4] and d["search_options"] == {**d["search_options"], "kernel": 4, "tile_group_w": 4}
+    assert "search_tiledq_kernel" in d["search_kernel"]
     assert "cpu_baseline" not in d
 
 

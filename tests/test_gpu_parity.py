@@ -253,6 +253,32 @@ def test_search_split_entry_point(kb, orc):
     assert_search_exact(g, orc.search(pp, times, vel, 4, 2))
 
 
+@pytest.mark.parametrize("which", KERNELS)
+def test_search_row_bands_concatenate_to_the_full_search(kb, orc, which):
+    """kbmod_search_rows ("entirely independent"): disjoint bands of
+    start rows of one stack, searched one after the other on this GPU, concatenate to the full
+    search bit for bit; the planes hold the band only; a prebuilt kbmod_plan gives the same."""
+    kb.set_search_kernel(which)
+    cfg = synth.config(2, N=8, H=75, W=203)
+    st = synth.make_stack(cfg)
+    pp = orc.make_psi_phi(st.sci, st.var, st.mask, st.psf)
+    d_pp = _cuda(pp)
+    full = _np(kb.search(d_pp, st.times, st.vel_grid, cfg.K, cfg.min_obs))
+    assert_search_exact(full, orc.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs))
+    from paper_1901_02492_b200 import shard
+    for world in (2, 3):
+        parts = [_np(kb.search(d_pp, st.times, st.vel_grid, cfg.K, cfg.min_obs, y_begin=y0, y_end=y1))
+                 for y0, y1 in shard.row_bands(cfg.H, world)]
+        cat = {k: np.concatenate([p[k] for p in parts], 0) for k in full}
+        assert_search_exact(cat, full)
+    plan = kb.Plan(st.times, cfg.N, cfg.H, cfg.W, st.vel_grid, cfg.K)
+    for y0, y1 in ((0, cfg.H), (31, 33), (74, 75), (40, 40)):
+        band = _np(kb.search(d_pp, None, None, cfg.K, cfg.min_obs, y_begin=y0, y_end=y1, plan=plan))
+        assert band["nu"].shape == (y1 - y0, cfg.W, cfg.K)
+        assert_search_exact(band, {k: v[y0:y1] for k, v in full.items()})
+    plan.close()
+
+
 def test_errors_are_loud(kb):
     pp = _cuda(synth.random_psiphi(2, 8, 8, seed=1))
     with pytest.raises(kb.KbmodError):

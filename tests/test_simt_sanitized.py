@@ -56,19 +56,22 @@ def test_the_detector_detects():
 
 @pytest.mark.skipif(os.environ.get("KBMOD_SIMT_SANITIZE") == "1", reason="already inside the sanitized child")
 def test_tiled_kernels_under_asan_ubsan():
-    """Kernels 2 and 4 (search_tiled.cu): config 1, crops, interior lists, degenerate shapes, image
-    counts, the limit cases and a seeded part of the randomized problems."""
+    """Kernels 2 and 4 (search_tiled.cu): config 1, the K = 16 crop, degenerate shapes, image counts,
+    the limit cases, row bands and the seeded randomized problems (about half a minute of emulation)."""
     _run_child(["tests/test_tiled_simt.py", "-k",
-                "config1 or crops or interior or degenerate or image_count or limit or randomized"])
+                "config1 or (crops and over2) or degenerate or image_count or limit or band or randomized"])
 
 
 @pytest.mark.skipif(os.environ.get("KBMOD_SIMT_SANITIZE") == "1", reason="already inside the sanitized child")
 def test_staged_kernel_under_asan_ubsan():
-    """Kernel 3 (search_staged.cu): config 1 under all schedules, crops, limit cases, ring geometries."""
-    _run_child(["tests/test_staged_simt.py", "-k", "config1 or crops or limit or geometr or degenerate"])
+    """Kernel 3 (search_staged.cu): config 1 under all schedules, the K = 16 crop, limit cases, row
+    bands, every ring geometry, literal-shift entries, image counts, randomized problems on ring 0."""
+    _run_child(["tests/test_staged_simt.py", "-k",
+                "config1 or (crops and over2) or limit or band or geometr or degenerate or unproven or image_count "
+                "or (randomized and 0)"])
 
 
 @pytest.mark.skipif(os.environ.get("KBMOD_SIMT_SANITIZE") == "1", reason="already inside the sanitized child")
 def test_oracle_under_asan_ubsan():
     """oracle.c itself with -fsanitize=address,undefined on the pins that exercise every function."""
-    _run_child(["tests/test_oracle_pins.py", "-k", "p4 or p5 or p6 or topk or asymmetric"])
+    _run_child(["tests/test_oracle_pins.py"])

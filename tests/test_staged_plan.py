@@ -50,11 +50,11 @@ def literal_pixels(p0, v, dt, n):
     return np.where(ok, g, 0).astype(np.int64), ok
 
 
-def run_plan(pp, times, vel, tiles=None):
+def run_plan(pp, times, vel, tiles=None, geom=0):
     """Interprets the plan for the given tiles; returns dict (tile_x, tile_y) -> Psi, Phi, n of
     shape [TH, TW, V] (only pixels inside the image are meaningful)."""
     N, H, W, _ = pp.shape
-    stream, shapes, info = binding.debug_staged_plan(times, N, H, W, vel)
+    stream, shapes, info = binding.debug_staged_plan(times, N, H, W, vel, geom)
     TW, TH, B = info["TW"], info["TH"], info["B"]
     enc = encode(pp)
     dt = (np.asarray(times, np.float64) - float(times[0])).astype(np.float32)
@@ -117,9 +117,9 @@ def run_plan(pp, times, vel, tiles=None):
     return out, info
 
 
-def check_against_oracle(orc, pp, times, vel, tiles=None):
+def check_against_oracle(orc, pp, times, vel, tiles=None, geom=0):
     N, H, W, _ = pp.shape
-    res, info = run_plan(pp, times, vel, tiles)
+    res, info = run_plan(pp, times, vel, tiles, geom)
     rPsi, rPhi, rn = orc.eval_all(pp, times, vel)           # [H, W, V], f32seq
     for (tile_x, tile_y), (Psi, Phi, cnt) in res.items():
         h, w = min(info["TH"], H - tile_y), min(info["TW"], W - tile_x)
@@ -142,16 +142,16 @@ def test_plan_reproduces_oracle_on_crops(orc, k, over):
     check_against_oracle(orc, pp, st.times, st.vel_grid)
 
 
-@pytest.mark.parametrize("geom", ["1", "2", "3", "6"])
-def test_plan_ring_geometry_variants(orc, geom, monkeypatch):
-    """KBMOD_STAGED_GEOM selects other slot sizes: the plan must stay exact and respect the cap."""
-    monkeypatch.setenv("KBMOD_STAGED_GEOM", geom)
+@pytest.mark.parametrize("geom", [1, 2, 3, 6])
+def test_plan_ring_geometry_variants(orc, geom):
+    """kbmod_search_options.staged_geom selects other slot sizes: the plan must stay exact and
+    respect the cap."""
     cfg = synth.config(3, N=15, H=70, W=133, n_sources=4)
     st = synth.make_stack(cfg)
     pp = orc.make_psi_phi(st.sci, st.var, st.mask, st.psf)
-    _, _, info = binding.debug_staged_plan(st.times, cfg.N, cfg.H, cfg.W, st.vel_grid)
-    assert info["CAP"] == {"1": 3072, "2": 6144, "3": 2560, "6": 8192}[geom]
-    check_against_oracle(orc, pp, st.times, st.vel_grid)
+    _, _, info = binding.debug_staged_plan(st.times, cfg.N, cfg.H, cfg.W, st.vel_grid, geom)
+    assert info["CAP"] == {1: 3072, 2: 6144, 3: 2560, 6: 8192}[geom]
+    check_against_oracle(orc, pp, st.times, st.vel_grid, geom=geom)
 
 
 def test_plan_interior_trajectories(orc):

@@ -38,18 +38,20 @@ def sim():
     return simt_build.load("staged_simt", '"simt_ptx.h"')
 
 
-def run_sim(sim, pp, times, vel, K, min_obs, order=0, seed=1, sms=3, tma_delay=0):
+def run_sim(sim, pp, times, vel, K, min_obs, order=0, seed=1, sms=3, tma_delay=0, geom=0, y_begin=0, y_end=None):
     """launch_search_staged under emulation; returns (status code, result planes, stats dict)."""
     N, H, W, _ = pp.shape
+    y_end = H if y_end is None else y_end
     pp = np.ascontiguousarray(pp, np.float32)
     times = np.ascontiguousarray(times, np.float64)
     vel = np.ascontiguousarray(vel, np.float32)
-    out = {k: np.full((H, W, K), -77, np.int32 if k in ("vel_idx", "n_obs") else np.float32) for k in PLANES}
+    out = {k: np.full((y_end - y_begin, W, K), -77, np.int32 if k in ("vel_idx", "n_obs") else np.float32)
+           for k in PLANES}
     stats = (ctypes.c_longlong * 8)()
     ptr = lambda a: a.ctypes.data_as(ctypes.c_void_p)
     rc = sim.simt_search_staged(ptr(pp), ptr(times), N, H, W, ptr(vel), int(vel.shape[0]), int(K), int(min_obs),
-                                *[ptr(out[k]) for k in PLANES], int(order), ctypes.c_uint(seed), int(sms),
-                                int(tma_delay), stats)
+                                int(y_begin), int(y_end), *[ptr(out[k]) for k in PLANES], int(geom), int(order),
+                                ctypes.c_uint(seed), int(sms), int(tma_delay), stats)
     names = ("smem_faults", "tma_loads", "tma_faults", "launches", "status")
     return rc, out, dict(zip(names, list(stats)))
 
@@ -102,15 +104,15 @@ def test_crops_of_the_baseline_configs(sim, orc, k, over):
     assert_exact(out, ref, stats, rc)
 
 
-@pytest.mark.parametrize("geom", ["1", "2", "3", "4", "5", "6"])
-def test_ring_geometries(sim, orc, geom, monkeypatch):
-    """Every ring geometry, fixed slots (1-3) and the byte-granular data ring (4-6)."""
-    monkeypatch.setenv("KBMOD_STAGED_GEOM", geom)
+@pytest.mark.parametrize("geom", [1, 2, 3, 4, 5, 6])
+def test_ring_geometries(sim, orc, geom):
+    """Every ring geometry (kbmod_search_options.staged_geom), fixed slots (1-3) and the
+    byte-granular data ring (4-6)."""
     pp = synth.random_psiphi(9, 64, 130, seed=21, invalid_frac=0.03)
     times = np.array([0, .05, .1, .15, 1, 1.05, 1.1, 2.0, 2.05])
     vel = synth.velocity_grid(8, 6, -math.pi / 3, math.pi / 3, 3.0, 40.0)
     ref = orc.search(pp, times, vel, 8, 4)
-    rc, out, stats = run_sim(sim, pp, times, vel, 8, 4, order=2, seed=int(geom), sms=2, tma_delay=60)
+    rc, out, stats = run_sim(sim, pp, times, vel, 8, 4, order=2, seed=geom, sms=2, tma_delay=60, geom=geom)
     assert_exact(out, ref, stats, rc)
 
 
@@ -183,6 +185,20 @@ def test_limit_cases(sim, orc):
     assert_exact(out, orc.search(pp, times, big, 4, 1), stats, rc)
 
 
+def test_row_bands_equal_the_full_search(sim, orc):
+    """kbmod_search_rows on the staged kernel: bands (tile-aligned or not, one row, empty, the last
+    rows) equal the same rows of the oracle's full search; the planes hold the band only."""
+    pp = synth.random_psiphi(5, 70, 90, seed=31, invalid_frac=0.1)
+    times = np.array([0.0, 0.3, 1.0, 1.4, 2.0])
+    vel = synth.velocity_grid(4, 3, -math.pi, math.pi, 1.0, 20.0)
+    full = orc.search(pp, times, vel, 4, 2)
+    for y0, y1 in ((0, 30), (30, 70), (5, 41), (69, 70), (17, 17), (0, 70)):
+        rc, out, stats = run_sim(sim, pp, times, vel, 4, 2, order=2, seed=y0 + 1, sms=2, tma_delay=9, y_begin=y0, y_end=y1)
+        if y1 == y0:
+            stats["launches"] += 1            # an empty band launches the encode kernel only
+        assert_exact(out, {k: v[y0:y1] for k, v in full.items()}, stats, rc)
+
+
 def test_image_count_variants(sim, orc):
     """N = 20 (one history register per pixel), N = 40 and N = 64 = KBMOD_MAX_IMAGES (additive counts)."""
     rng = np.random.default_rng(64)
@@ -195,15 +211,14 @@ def test_image_count_variants(sim, orc):
         assert_exact(out, ref, stats, rc)
 
 
-@pytest.mark.parametrize("geom", ["0", "5"])
-def test_randomized_shapes(sim, orc, geom, monkeypatch):
+@pytest.mark.parametrize("geom", [0, 5])
+def test_randomized_shapes(sim, orc, geom):
     """25 seeded random problems per ring kind, random schedule, CTA count and TMA delay (a longer
     run of the same generator, 2 025 cases on geometries 0 and 4, found no mismatch)."""
     from tests.test_tiled_simt import random_case
-    monkeypatch.setenv("KBMOD_STAGED_GEOM", geom)
-    rng = np.random.default_rng(77 + int(geom))
+    rng = np.random.default_rng(77 + geom)
     for _ in range(25):
         pp, times, vel, K, mo = random_case(rng)
         rc, out, stats = run_sim(sim, pp, times, vel, K, mo, int(rng.integers(3)), int(rng.integers(1 << 30)),
-                                 int(rng.integers(1, 5)), int(rng.choice([0, 10, 100])))
+                                 int(rng.integers(1, 5)), int(rng.choice([0, 10, 100])), geom=geom)
         assert_exact(out, orc.search(pp, times, vel, K, mo), stats, rc)

@@ -32,18 +32,21 @@ def sim():
     return simt_build.load("tiled_simt", '1')
 
 
-def run_sim(sim, pp, times, vel, K, min_obs, queued, order=0, seed=1):
+def run_sim(sim, pp, times, vel, K, min_obs, queued, order=0, seed=1, y_begin=0, y_end=None, group_w=0):
     N, H, W, _ = pp.shape
+    y_end = H if y_end is None else y_end
     pp = np.ascontiguousarray(pp, np.float32)
     times = np.ascontiguousarray(times, np.float64)
     vel = np.ascontiguousarray(vel, np.float32)
-    out = {k: np.full((H, W, K), -77, np.int32 if k in ("vel_idx", "n_obs") else np.float32) for k in PLANES}
+    out = {k: np.full((y_end - y_begin, W, K), -77, np.int32 if k in ("vel_idx", "n_obs") else np.float32)
+           for k in PLANES}
     stats = (ctypes.c_longlong * 8)()
     ptr = lambda a: a.ctypes.data_as(ctypes.c_void_p)
     rc = sim.simt_search_tiled(ptr(pp), ptr(times), N, H, W, ptr(vel), int(vel.shape[0]), int(K), int(min_obs),
-                               *[ptr(out[k]) for k in PLANES], int(queued), int(order), ctypes.c_uint(seed), stats)
+                               int(y_begin), int(y_end), *[ptr(out[k]) for k in PLANES], int(queued), int(group_w),
+                               int(order), ctypes.c_uint(seed), stats)
     assert rc == 0, f"launch_search_tiled returned {rc}"
-    assert stats[3] == 2, "encode kernel + search kernel"
+    assert stats[3] == (2 if y_end > y_begin else 1), "encode kernel + search kernel"
     return out
 
 
@@ -202,10 +205,22 @@ def test_queued_randomized_shapes(sim, orc):
         assert_exact(out, orc.search(pp, times, vel, K, mo))
 
 
-@pytest.mark.parametrize("gw", ["1", "3", "200"])
-def test_queued_tile_order_knob_does_not_change_results(sim, orc, gw, monkeypatch):
-    """KBMOD_TILED_GROUPW only permutes which CTA takes which tile (bench.py sweeps it for speed)."""
-    monkeypatch.setenv("KBMOD_TILED_GROUPW", gw)
+@pytest.mark.parametrize("gw", [1, 3, 200])
+def test_queued_tile_order_knob_does_not_change_results(sim, orc, gw):
+    """kbmod_search_options.tile_group_w only permutes which CTA takes which tile."""
     cfg, st, pp = stack_case(orc, 3, N=15, H=70, W=300, n_sources=4)        # 5 x 3 tiles, ragged on both axes
     ref = orc.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs)
-    assert_exact(run_sim(sim, pp, st.times, st.vel_grid, cfg.K, cfg.min_obs, QUEUED, order=2, seed=int(gw)), ref)
+    assert_exact(run_sim(sim, pp, st.times, st.vel_grid, cfg.K, cfg.min_obs, QUEUED, order=2, seed=gw, group_w=gw), ref)
+
+
+@pytest.mark.parametrize("queued", [TILED, QUEUED])
+def test_row_bands_equal_the_full_search(sim, orc, queued):
+    """kbmod_search_rows: bands of start rows (tile-aligned or not, one row, empty, the last rows)
+    equal the same rows of the oracle's full search; the planes hold the band only."""
+    pp = synth.random_psiphi(5, 70, 90, seed=31, invalid_frac=0.1)
+    times = np.array([0.0, 0.3, 1.0, 1.4, 2.0])
+    vel = synth.velocity_grid(4, 3, -math.pi, math.pi, 1.0, 20.0)
+    full = orc.search(pp, times, vel, 4, 2)
+    for y0, y1 in ((0, 32), (32, 70), (5, 41), (69, 70), (17, 17), (0, 70)):
+        out = run_sim(sim, pp, times, vel, 4, 2, queued, order=2, seed=y0 + 1, y_begin=y0, y_end=y1)
+        assert_exact(out, {k: v[y0:y1] for k, v in full.items()})
