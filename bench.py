@@ -18,7 +18,9 @@ kbmod_search_options; the host plan (kbmod_plan: it depends on times / grid / sh
 once before the timed region, as a survey pipeline searching many stacks of one cadence would.
 
 N > 1 (torchrun): every rank searches its own independent stack (the survey's fields/CCDs are
-independent searches) -- weak scaling, no data-path collective.
+independent searches) -- weak scaling, no data-path collective.  --bands (N > 1):
+ONE stack replicated on every rank, each rank searching its band of start rows through
+kbmod_search_rows -- strong scaling, still no data-path collective.
 """
 import argparse
 import json
@@ -189,7 +191,8 @@ def config_dict(cfg, args):
             "trajectories": cfg.trajectories, "trajectory_evals": cfg.evals,
             "step": "kbmod_make_psi_phi + kbmod_search (S1..S6)",
             "l2": "inputs larger than L2 (stack 2.0 GB+ vs 126 MB); no flush needed",
-            "parallelism": f"independent stacks x{args.gpus}"}
+            "parallelism": (f"one stack, start-row bands x{args.gpus} (kbmod_search_rows)" if getattr(args, "bands", False)
+                            and args.gpus > 1 else f"independent stacks x{args.gpus}")}
 
 
 # ----------------------------------------------------------------------------------------------
@@ -217,21 +220,23 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     h_mask = torch.from_numpy(st.mask).pin_memory()
     d_sci, d_var, d_mask = h_sci.to(dev), h_var.to(dev), h_mask.to(dev)
     psiphi = torch.empty((N, H, W, 2), dtype=torch.float32, device=dev)
-    out = binding.alloc_result(H, W, K, dev)
+    bands = bool(args.bands) and world > 1
+    y0, y1 = shard.row_bands(H, world)[rank] if bands else (0, H)
+    out = binding.alloc_result(y1 - y0, W, K, dev)
     ws = torch.empty(binding.search_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
     h_out = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
     e_sci, e_var, e_mask = torch.empty_like(d_sci), torch.empty_like(d_var), torch.empty_like(d_mask)
 
     def step_resident():
         binding.make_psi_phi(d_sci, d_var, d_mask, st.psf, out=psiphi)
-        binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan)
+        binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan, y_begin=y0, y_end=y1)
 
     def step_e2e():
         e_sci.copy_(h_sci, non_blocking=True)
         e_var.copy_(h_var, non_blocking=True)
         e_mask.copy_(h_mask, non_blocking=True)
         binding.make_psi_phi(e_sci, e_var, e_mask, st.psf, out=psiphi)
-        binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan)
+        binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan, y_begin=y0, y_end=y1)
         for k in out:
             h_out[k].copy_(out[k], non_blocking=True)
 
@@ -278,7 +283,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     reps = max(3, min(args.steps, 10))
     ms_psiphi = phase(lambda: binding.make_psi_phi(d_sci, d_var, d_mask, st.psf, out=psiphi), reps)
     ms_search = phase(lambda: binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws,
-                                             plan=plan), reps)
+                                             plan=plan, y_begin=y0, y_end=y1), reps)
 
     binding.search_status(ws)
     step_e2e()
@@ -311,13 +316,14 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     if rank != 0:
         return
     hbm_gbs, sm_max_mhz, peak_src = load_peaks()
-    evals = cfg.evals * world
+    evals = cfg.evals * (1 if bands else world)        # --bands: one stack shared by all ranks
     ms_per_step = total_ms / args.steps
     value = evals / (ms_per_step * 1e-3)
     # roofline of the dominant kernel (the search): algorithmic shared-memory sample bytes
     # (8 B per trajectory-eval) against the LSU peak 148 SM x 128 B/clk x max SM clock
     lsu_peak = SM_COUNT * LDS_BYTES_PER_CLK_PER_SM * sm_max_mhz * 1e6 / 1e9       # GB/s
-    achieved = cfg.evals * SAMPLE_BYTES / (ms_search * 1e-3) / 1e9
+    band_evals = cfg.evals * (y1 - y0) // H           # what THIS rank's search launch processed
+    achieved = band_evals * SAMPLE_BYTES / (ms_search * 1e-3) / 1e9
     hbm_bytes = N * H * W * 8 + H * W * K * 24
     # e2e: host buffers in, host result planes out, transfers inside the timed region.  The headline
     # is the single C-ABI call on HOST buffers (kbmod_search_host) when its planes were verified
@@ -335,9 +341,9 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "scaling": "strong" if bands else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": config_dict(cfg, args),
-        "trajectories_per_s": cfg.trajectories * world / (ms_per_step * 1e-3),
+        "trajectories_per_s": cfg.trajectories * (1 if bands else world) / (ms_per_step * 1e-3),
         "phases_ms": {"make_psi_phi": ms_psiphi, "search": ms_search},
         "search_only": {"trajectory_evals_per_s": cfg.evals / (ms_search * 1e-3),
                         "trajectories_per_s": cfg.trajectories / (ms_search * 1e-3)},
@@ -353,7 +359,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
                      "hbm": {"compulsory_bytes": hbm_bytes, "peak": hbm_gbs,
                              "achieved": hbm_bytes / (ms_search * 1e-3) / 1e9,
                              "floor_ms": hbm_bytes / (hbm_gbs * 1e9) * 1e3},
-                     "lsu_floor_ms": cfg.evals * SAMPLE_BYTES / (lsu_peak * 1e9) * 1e3},
+                     "lsu_floor_ms": band_evals * SAMPLE_BYTES / (lsu_peak * 1e9) * 1e3},
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": e2e,
         "e2e_binding_copies": e2e_binding,
@@ -388,6 +394,8 @@ def main():
                          "3 TMA-staged, 4 tiled + queued top-K (3 and 4: opt-in, see DESIGN.md section 8)")
     ap.add_argument("--group-w", type=int, default=0, help="kbmod_search_options.tile_group_w (0 = default)")
     ap.add_argument("--staged-geom", type=int, default=0, help="kbmod_search_options.staged_geom (kernel 3)")
+    ap.add_argument("--bands", action="store_true",
+                    help="N > 1: one replicated stack, one band of start rows per rank (strong scaling)")
     ap.add_argument("--ref-rows", type=int, default=256, help="start rows per oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
@@ -408,7 +416,8 @@ def main():
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl")
-    st = synth.make_stack(cfg, seed=shard.rank_seed(cfg.seed, rank))     # an independent stack per rank
+    # an independent stack per rank (weak scaling), or the same stack on every rank (--bands)
+    st = synth.make_stack(cfg, seed=cfg.seed if args.bands else shard.rank_seed(cfg.seed, rank))
     run_gpu(args, cfg, st, rank, world, local_rank)
     if world > 1:
         dist.destroy_process_group()

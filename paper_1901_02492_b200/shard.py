@@ -8,7 +8,7 @@ GPUs, gloo in the CPU tests); every function degrades to the single-process case
 """
 from __future__ import annotations
 
-from typing import Dict, List, Tuple
+from typing import Callable, Dict, List, Optional, Tuple
 
 import torch
 import torch.distributed as dist
@@ -73,3 +73,20 @@ def gather_bands(band: Dict[str, torch.Tensor], H: int) -> Dict[str, torch.Tenso
         dist.all_gather(parts, pad)
         out[k] = torch.cat([p[: y1 - y0] for p, (y0, y1) in zip(parts, bands)], 0)
     return out
+
+
+def search_row_band(psiphi, times, vel_grid, K: int, min_obs: int, search: Optional[Callable] = None,
+                    gather: bool = True, **kw) -> Dict[str, torch.Tensor]:
+    """One stack, replicated on every rank, searched in start-row bands:
+    this rank runs kbmod_search_rows on its band of row_bands(H, world) and, if `gather`, the bands
+    are concatenated into [H, W, K] planes on every rank.  No collective on the data path of the
+    search itself.  `search` defaults to binding.search (the C-ABI call); the CPU tests pass the
+    same call of the SIMT-emulated library."""
+    if search is None:
+        from . import binding
+        search = binding.search
+    rank, n = world()
+    H = int(psiphi.shape[1])
+    y0, y1 = row_bands(H, n)[rank]
+    band = search(psiphi, times, vel_grid, K, min_obs, y_begin=y0, y_end=y1, **kw)
+    return gather_bands(band, H) if gather else band

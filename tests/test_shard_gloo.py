@@ -1,7 +1,8 @@
 """N > 1 host logic on CPU: world_size 2, gloo.  Each rank searches its band of start rows of one
-replicated stack with the oracle standing in for the per-GPU search (the test is about the
-partition, the gather and the timing reduction, not the kernels); the concatenated planes must
-equal a single-process search, and the step time must be the slowest rank's."""
+replicated stack through shard.search_row_band, whose per-rank search is the PRODUCT's band call
+(launch_search_tiled with y_begin / y_end, the code behind kbmod_search_rows) run under the SIMT
+emulator of tests/hostlogic/ in place of a GPU; the concatenated planes must equal the oracle's
+single-process search bit for bit, and the step time must be the slowest rank's."""
 import os
 import socket
 
@@ -31,10 +32,15 @@ def _worker(rank, world, port, ret):
         pp = synth.random_psiphi(4, 23, 40, seed=11, invalid_frac=0.05)     # same stack on every rank
         vel = synth.velocity_grid(4, 3, -1.0, 1.0, 2.0, 9.0)
         times = [0.0, 0.4, 1.0, 1.5]
-        y0, y1 = shard.row_bands(23, world)[rank]
-        res = oracle.search(pp, times, vel, 3, 2, y_begin=y0, y_end=y1)
-        band = {k: torch.from_numpy(np.ascontiguousarray(v)) for k, v in res.items()}
-        full = shard.gather_bands(band, 23)
+        from tests import simt_build, test_tiled_simt as T
+        sim = simt_build.load("tiled_simt", "1")
+
+        def emulated_search(psiphi, times, vel_grid, K, min_obs, y_begin, y_end):
+            out = T.run_sim(sim, psiphi.numpy(), times, vel_grid, K, min_obs, T.QUEUED if rank else T.TILED,
+                            order=2, seed=rank + 1, y_begin=y_begin, y_end=y_end)
+            return {k: torch.from_numpy(v) for k, v in out.items()}
+
+        full = shard.search_row_band(torch.from_numpy(pp), times, vel, 3, 2, search=emulated_search)
         ref = oracle.search(pp, times, vel, 3, 2)
         for k in ref:
             a, b = full[k].numpy(), ref[k]
@@ -66,6 +72,8 @@ def test_world_size_2_gloo(orc):
     ctx = mp.get_context("spawn")
     ret = ctx.Manager().dict()
     port = _free_port()
+    from tests import simt_build
+    simt_build.load("tiled_simt", "1")            # compile once, before the ranks race for it
     procs = [ctx.Process(target=_worker, args=(r, 2, port, ret)) for r in range(2)]
     for p in procs:
         p.start()
