@@ -158,3 +158,87 @@ def score(Psi, Phi):
     if rc != 0:
         raise ValueError(f"oracle_score failed: {rc}")
     return nu, alpha
+
+
+# ----------------------------------------------------------------------------- next rows (N1..N4)
+def search_threshold(psiphi, times, vel_grid, min_obs, nu_min, y_begin=0, y_end=None, capacity=1 << 22):
+    """N4 -> (count, dict of arrays [min(count, capacity)]: x, y, vel_idx, n_obs, psi, phi, nu, alpha),
+    in (y0, x0, j) order."""
+    psiphi = _c(psiphi, np.float32)
+    times = _c(times, np.float64)
+    vel = _c(vel_grid, np.float32)
+    N, H, W, _ = psiphi.shape
+    y_end = H if y_end is None else y_end
+    ints = {k: np.zeros(capacity, np.int32) for k in ("x", "y", "vel_idx", "n_obs")}
+    flts = {k: np.zeros(capacity, np.float32) for k in ("psi", "phi", "nu", "alpha")}
+    fn = lib().oracle_search_threshold
+    fn.restype = ctypes.c_longlong
+    n = fn(_p(psiphi), _p(times), N, H, W, _p(vel), int(vel.shape[0]), int(min_obs), ctypes.c_float(nu_min),
+           int(y_begin), int(y_end), ctypes.c_longlong(capacity), _p(ints["x"]), _p(ints["y"]),
+           _p(ints["vel_idx"]), _p(ints["n_obs"]), _p(flts["psi"]), _p(flts["phi"]), _p(flts["nu"]),
+           _p(flts["alpha"]))
+    if n < 0:
+        raise ValueError(f"oracle_search_threshold failed: {n}")
+    k = min(int(n), capacity)
+    return int(n), {**{a: v[:k] for a, v in ints.items()}, **{a: v[:k] for a, v in flts.items()}}
+
+
+def filter_candidates(psiphi, times, x0y0, vxvy, sigma_reject=5.0, q=0.0):
+    """N1 -> dict: psi, phi, nu, alpha [M] f32, n_obs [M] i32, keep [M] u64, kalman [M,2] f32."""
+    psiphi = _c(psiphi, np.float32)
+    times = _c(times, np.float64)
+    x0y0 = _c(x0y0, np.int32).reshape(-1, 2)
+    vxvy = _c(vxvy, np.float32).reshape(-1, 2)
+    N, H, W, _ = psiphi.shape
+    M = x0y0.shape[0]
+    out = {k: np.zeros(M, np.float32) for k in ("psi", "phi", "nu", "alpha")}
+    out["n_obs"] = np.zeros(M, np.int32)
+    out["keep"] = np.zeros(M, np.uint64)
+    out["kalman"] = np.zeros((M, 2), np.float32)
+    lib().oracle_filter_candidates.restype = ctypes.c_int
+    rc = lib().oracle_filter_candidates(_p(psiphi), _p(times), N, H, W, _p(x0y0), _p(vxvy), M,
+                                        ctypes.c_float(sigma_reject), ctypes.c_float(q), _p(out["psi"]),
+                                        _p(out["phi"]), _p(out["n_obs"]), _p(out["nu"]), _p(out["alpha"]),
+                                        _p(out["keep"]), _p(out["kalman"]))
+    if rc != 0:
+        raise ValueError(f"oracle_filter_candidates failed: {rc}")
+    return out
+
+
+def build_mask(sci, var, mask_in=None, sigma_thr=5.0, grow=2, min_images=2, bright_counts=120.0):
+    """N3 -> mask [N,H,W] u8."""
+    sci = _c(sci, np.float32)
+    var = _c(var, np.float32)
+    N, H, W = sci.shape
+    if mask_in is not None:
+        mask_in = _c(mask_in, np.uint8)
+    out = np.zeros((N, H, W), np.uint8)
+    lib().oracle_build_mask.restype = ctypes.c_int
+    rc = lib().oracle_build_mask(_p(sci), _p(var), _p(mask_in), N, H, W, ctypes.c_float(sigma_thr), int(grow),
+                                 int(min_images), ctypes.c_float(bright_counts), _p(out))
+    if rc != 0:
+        raise ValueError(f"oracle_build_mask failed: {rc}")
+    return out
+
+
+def coadd_stamps(sci, mask, times, x0y0, vxvy, keep=None, R=10):
+    """N2 -> stamps [M,2R+1,2R+1] f32, moments [M,6] f32 (m00, cx, cy, mu20, mu02, mu11)."""
+    sci = _c(sci, np.float32)
+    times = _c(times, np.float64)
+    x0y0 = _c(x0y0, np.int32).reshape(-1, 2)
+    vxvy = _c(vxvy, np.float32).reshape(-1, 2)
+    N, H, W = sci.shape
+    M = x0y0.shape[0]
+    if mask is not None:
+        mask = _c(mask, np.uint8)
+    if keep is not None:
+        keep = _c(keep, np.uint64)
+    S = 2 * R + 1
+    stamps = np.zeros((M, S, S), np.float32)
+    moments = np.zeros((M, 6), np.float32)
+    lib().oracle_coadd_stamps.restype = ctypes.c_int
+    rc = lib().oracle_coadd_stamps(_p(sci), _p(mask), _p(times), N, H, W, _p(x0y0), _p(vxvy), _p(keep), M, int(R),
+                                   _p(stamps), _p(moments))
+    if rc != 0:
+        raise ValueError(f"oracle_coadd_stamps failed: {rc}")
+    return stamps, moments
