@@ -107,7 +107,7 @@ typedef struct {
     int32_t kernel;         /* KBMOD_KERNEL_* */
     int32_t tile_group_w;   /* kernels 2, 4: tile columns per rasterisation group, 1..256; 0 = default.
                                Changes which CTA takes which tile, never the results */
-    int32_t staged_geom;    /* kernel 3: shared-memory ring geometry 0..6 (csrc/search_staged.cu) */
+    int32_t staged_geom;    /* kernel 3: shared-memory ring geometry 0..3 (csrc/search_staged.cu) */
 } kbmod_search_options;
 
 /*
@@ -170,6 +170,92 @@ int kbmod_plan_kernel(const kbmod_plan* plan);
 int kbmod_search_planned(const kbmod_plan* plan, const float* psiphi, int min_obs, int y_begin, int y_end,
                          const kbmod_result* out, void* workspace, size_t workspace_bytes, void* stream);
 void kbmod_plan_destroy(kbmod_plan* plan);
+
+/*
+ * Threshold-mode search: the paper's own retention rule ("evaluate nu for all possible values
+ * of y0 and v, and examine those that are above a desired detection threshold"; threshold
+ * 10).  Same S3, S4, S5 and eligibility as kbmod_search; instead of the K best per start pixel,
+ * EVERY eligible trajectory of the band with nu >= nu_min is appended to a compacted candidate list
+ * (start pixel, velocity index, n_obs, Psi, Phi, nu, alpha).  There is no dense [H][W][K] output.
+ *   out      : HOST struct of DEVICE arrays of `capacity` elements each, caller-owned
+ *   count    : DEVICE counter; set to the number of trajectories found.  If it exceeds `capacity`
+ *              only `capacity` of them were stored (which ones is unspecified) -- enlarge and rerun.
+ *   The order of the list is unspecified; its content (as a set) is exactly the definition's.
+ *   options  : kernel AUTO / DIRECT = the direct-gather kernel; TILED_QUEUED = the tiled gathers
+ *              with the queue-compacted epilogue; TILED and STAGED: KBMOD_ERR_UNSUPPORTED.
+ *   workspace: as kbmod_search with K = 8 (kbmod_search_workspace(N,H,W,V,8))
+ */
+typedef struct {
+    int32_t* x;        /* start pixel */
+    int32_t* y;
+    int32_t* vel_idx;
+    int32_t* n_obs;
+    float* psi;
+    float* phi;
+    float* nu;
+    float* alpha;
+} kbmod_candidates;
+
+int kbmod_search_threshold(const float* psiphi, const double* times, int N, int H, int W,
+                           const float* vel_grid, int V, int min_obs, float nu_min, int y_begin, int y_end,
+                           const kbmod_candidates* out, long long capacity, unsigned long long* count,
+                           void* workspace, size_t workspace_bytes, const kbmod_search_options* options,
+                           void* stream);
+
+/*
+ * Light-curve outlier filter and re-score of candidate trajectories (section 3.3: "a variation
+ * on the Kalman filter ... filter out any observations that are more than five standard deviations
+ * away from the best fit Kalman flux at that observation and use the remaining observations to
+ * recalculate the likelihood").  The paper gives no gains or noise model; this call implements the
+ * reading DESIGN.md N1-a..N1-e: light curve f_i = Psi_i/Phi_i with variance 1/Phi_i over the
+ * observations that exist (S3/S4) and have Phi_i > 0; a scalar Kalman filter (state = flux,
+ * random-walk process variance `process_var` per step) run forward and backward, the first
+ * observation of a pass initialises it, an observation is an outlier of the pass iff
+ * (f_i - x)^2 > sigma_reject^2 * (P + process_var + 1/Phi_i) and is then not ingested; the pass that
+ * keeps more observations decides (tie: forward); Psi, Phi, n_obs, nu, alpha are recomputed over
+ * the kept observations in image order (fp32, as kbmod_search).  All in separately rounded fp32.
+ *   x0y0 : [M][2] int32 device (start pixel);  vxvy : [M][2] float device (px/day), 8-byte aligned
+ *   psi, phi, nu, alpha : [M] float device;  n_obs : [M] int32 device
+ *   keep : [M] uint64 device, bit i = observation i exists and was kept
+ *   kalman : [M][2] float device or NULL: (flux estimate, variance) of the deciding pass
+ *   nu = -INFINITY, alpha = 0 when nothing is left or Phi <= 0.
+ */
+int kbmod_filter_candidates(const float* psiphi, const double* times, int N, int H, int W,
+                            const int32_t* x0y0, const float* vxvy, int M, float sigma_reject,
+                            float process_var, float* psi, float* phi, int32_t* n_obs, float* nu,
+                            float* alpha, uint64_t* keep, float* kalman, void* stream);
+
+/*
+ * Coadded postage stamps of candidate trajectories and their central moments (section 3.3:
+ * "coadded postage stamps ... central moments of the images ... similarity of the moments to a
+ * Gaussian centered at the middle of the stamp").  Reading DESIGN.md N2-a..N2-c:
+ *   stamp[dy][dx], dy, dx in [-R, R] = mean over the observations i of the trajectory (those with
+ *       bit i of keep[m] set; all when keep is NULL) of sci_i[iy_i+dy][ix_i+dx], over the images
+ *       where that pixel is inside the image, unmasked and finite; 0 where none contributes.
+ *   moments = (m00, cx, cy, mu20, mu02, mu11) of max(stamp, 0): total, centroid relative to the
+ *       stamp centre, central second moments; all zero when m00 <= 0.
+ * The accept/reject thresholds on the moments are the caller's (the paper gives none).
+ *   sci : [N][H][W] float device;  mask : [N][H][W] uint8 device or NULL;  R : 0..15
+ *   stamps : [M][2R+1][2R+1] float device;  moments : [M][6] float device or NULL
+ */
+int kbmod_coadd_stamps(const float* sci, const uint8_t* mask, const double* times, int N, int H, int W,
+                       const int32_t* x0y0, const float* vxvy, const uint64_t* keep, int M, int R,
+                       float* stamps, float* moments, void* stream);
+
+/*
+ * Mask builder (section 3.2; section 5.2).  A pixel of image i is detected iff sci
+ * and var are finite, var > 0 and sci > sigma_thr * sqrt(var) (background 0); detections are grown
+ * by the disc dx^2 + dy^2 <= grow^2 ("grown by an additional two pixels"); a pixel is static iff it
+ * is grown-detected in at least min_images images ("must be masked in at least one of the other
+ * science images"); mask_out_i = mask_in_i | static | (sci_i finite and > bright_counts) ("any
+ * pixel in any image that exceeded 120 counts").  The paper's footprint detection is the LSST
+ * stack's and is not described: this thresholding is reading DESIGN.md N3-a..N3-c.
+ *   sci, var : [N][H][W] float device;  mask_in : [N][H][W] uint8 device or NULL
+ *   grow : 0..8;  min_images >= 1;  mask_out : [N][H][W] uint8 device (may alias mask_in)
+ */
+int kbmod_build_mask(const float* sci, const float* var, const uint8_t* mask_in, int N, int H, int W,
+                     float sigma_thr, int grow, int min_images, float bright_counts,
+                     uint8_t* mask_out, void* stream);
 
 /* Completion status of the last kbmod_search that used this workspace.  SYNCHRONISES the stream
  * (the one call of the library that does).  KBMOD_OK, or KBMOD_ERR_TIMEOUT if a warp of the

@@ -21,8 +21,10 @@ EXPORTS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_rows", "kbmod_sea
            "kbmod_search_split", "kbmod_plan_create", "kbmod_plan_kernel", "kbmod_search_planned",
            "kbmod_plan_destroy", "kbmod_eval_trajectories", "kbmod_launch_count", "kbmod_status_string",
            "kbmod_version", "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host",
-           "kbmod_search_host_workspace")
-_INT_CALLS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_rows", "kbmod_search_split",
+           "kbmod_search_host_workspace", "kbmod_search_threshold", "kbmod_filter_candidates",
+           "kbmod_coadd_stamps", "kbmod_build_mask")
+_INT_CALLS = ("kbmod_search_threshold", "kbmod_filter_candidates", "kbmod_coadd_stamps", "kbmod_build_mask",
+              "kbmod_make_psi_phi", "kbmod_search", "kbmod_search_rows", "kbmod_search_split",
               "kbmod_plan_create", "kbmod_plan_kernel", "kbmod_search_planned", "kbmod_eval_trajectories",
               "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host")
 KERNEL_AUTO, KERNEL_DIRECT, KERNEL_TILED, KERNEL_STAGED, KERNEL_TILED_QUEUED = range(5)
@@ -34,6 +36,10 @@ class KbmodError(RuntimeError):
 
 class _Result(ctypes.Structure):
     _fields_ = [(n, ctypes.c_void_p) for n in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")]
+
+
+class _Candidates(ctypes.Structure):       # kbmod_candidates
+    _fields_ = [(n, ctypes.c_void_p) for n in ("x", "y", "vel_idx", "n_obs", "psi", "phi", "nu", "alpha")]
 
 
 class _Options(ctypes.Structure):          # kbmod_search_options
@@ -347,3 +353,98 @@ def eval_trajectories(psiphi: torch.Tensor, times, x0y0: torch.Tensor, vxvy: tor
                                        _dev(ixiy, torch.int32, "ixiy"), _stream())
     _check(rc, "kbmod_eval_trajectories")
     return Psi, Phi, nobs, ixiy
+
+
+# ----------------------------------------------------------------------------- rows around the search
+_CAND_INT, _CAND_FLT = ("x", "y", "vel_idx", "n_obs"), ("psi", "phi", "nu", "alpha")
+
+
+def search_threshold(psiphi: torch.Tensor, times, vel_grid, min_obs: int, nu_min: float, capacity: int,
+                     y_begin: int = 0, y_end: Optional[int] = None, kernel: Optional[int] = None,
+                     tile_group_w: int = 0, workspace: Optional[torch.Tensor] = None):
+    """kbmod_search_threshold -> (count tensor [1] uint64-as-int64 on the device, dict of device arrays
+    [capacity]: x, y, vel_idx, n_obs, psi, phi, nu, alpha).  The first min(count, capacity) entries
+    are valid, in unspecified order."""
+    N, H, W, two = psiphi.shape
+    if two != 2:
+        raise KbmodError("psiphi must be [N,H,W,2]")
+    times = _host(times, np.float64)
+    vel = _host(vel_grid, np.float32)
+    if times.shape != (N,) or vel.ndim != 2 or vel.shape[1] != 2:
+        raise KbmodError("times must be [N], vel_grid [V,2]")
+    V = vel.shape[0]
+    y_end = H if y_end is None else int(y_end)
+    dev = psiphi.device
+    out = {k: torch.empty(max(1, int(capacity)), dtype=torch.int32, device=dev) for k in _CAND_INT}
+    out.update({k: torch.empty(max(1, int(capacity)), dtype=torch.float32, device=dev) for k in _CAND_FLT})
+    count = torch.zeros(1, dtype=torch.int64, device=dev)
+    if workspace is None:
+        workspace = torch.empty(search_workspace(N, H, W, V, 8), dtype=torch.uint8, device=dev)
+    cand = _Candidates(*[ctypes.c_void_p(out[k].data_ptr()) for k in _CAND_INT + _CAND_FLT])
+    opt = _options(kernel, tile_group_w)
+    rc = lib().kbmod_search_threshold(_dev(psiphi, torch.float32, "psiphi"), times.ctypes.data_as(ctypes.c_void_p),
+                                      N, H, W, vel.ctypes.data_as(ctypes.c_void_p), V, int(min_obs),
+                                      ctypes.c_float(nu_min), int(y_begin), y_end, ctypes.byref(cand),
+                                      ctypes.c_longlong(int(capacity)), ctypes.c_void_p(count.data_ptr()),
+                                      _dev(workspace, torch.uint8, "workspace"), ctypes.c_size_t(workspace.numel()),
+                                      ctypes.byref(opt), _stream())
+    _check(rc, "kbmod_search_threshold")
+    return count, out
+
+
+def filter_candidates(psiphi: torch.Tensor, times, x0y0: torch.Tensor, vxvy: torch.Tensor,
+                      sigma_reject: float = 5.0, process_var: float = 0.0) -> Dict[str, torch.Tensor]:
+    """kbmod_filter_candidates -> dict: psi, phi, nu, alpha [M] f32, n_obs [M] i32, keep [M] i64 (the
+    uint64 bit mask), kalman [M,2] f32."""
+    N, H, W, _ = psiphi.shape
+    times = _host(times, np.float64)
+    M = int(x0y0.shape[0])
+    dev = psiphi.device
+    out = {k: torch.empty(M, dtype=torch.float32, device=dev) for k in ("psi", "phi", "nu", "alpha")}
+    out["n_obs"] = torch.empty(M, dtype=torch.int32, device=dev)
+    out["keep"] = torch.empty(M, dtype=torch.int64, device=dev)
+    out["kalman"] = torch.empty((M, 2), dtype=torch.float32, device=dev)
+    if tuple(x0y0.shape) != (M, 2) or tuple(vxvy.shape) != (M, 2) or times.shape != (N,):
+        raise KbmodError("x0y0, vxvy must be [M,2], times [N]")
+    rc = lib().kbmod_filter_candidates(_dev(psiphi, torch.float32, "psiphi"), times.ctypes.data_as(ctypes.c_void_p),
+                                       N, H, W, _dev(x0y0, torch.int32, "x0y0"), _dev(vxvy, torch.float32, "vxvy"), M,
+                                       ctypes.c_float(sigma_reject), ctypes.c_float(process_var),
+                                       *[ctypes.c_void_p(out[k].data_ptr()) for k in
+                                         ("psi", "phi", "n_obs", "nu", "alpha", "keep", "kalman")], _stream())
+    _check(rc, "kbmod_filter_candidates")
+    return out
+
+
+def coadd_stamps(sci: torch.Tensor, mask: Optional[torch.Tensor], times, x0y0: torch.Tensor, vxvy: torch.Tensor,
+                 keep: Optional[torch.Tensor] = None, R: int = 10):
+    """kbmod_coadd_stamps -> stamps [M,2R+1,2R+1] f32, moments [M,6] f32 (m00, cx, cy, mu20, mu02, mu11)."""
+    N, H, W = sci.shape
+    times = _host(times, np.float64)
+    M = int(x0y0.shape[0])
+    S = 2 * int(R) + 1
+    if tuple(x0y0.shape) != (M, 2) or tuple(vxvy.shape) != (M, 2) or times.shape != (N,):
+        raise KbmodError("x0y0, vxvy must be [M,2], times [N]")
+    if (mask is not None and mask.shape != sci.shape) or (keep is not None and tuple(keep.shape) != (M,)):
+        raise KbmodError("mask must match sci, keep must be [M]")
+    stamps = torch.empty((M, S, S), dtype=torch.float32, device=sci.device)
+    moments = torch.empty((M, 6), dtype=torch.float32, device=sci.device)
+    rc = lib().kbmod_coadd_stamps(_dev(sci, torch.float32, "sci"), _dev(mask, torch.uint8, "mask"),
+                                  times.ctypes.data_as(ctypes.c_void_p), N, H, W, _dev(x0y0, torch.int32, "x0y0"),
+                                  _dev(vxvy, torch.float32, "vxvy"), _dev(keep, torch.int64, "keep"), M, int(R),
+                                  ctypes.c_void_p(stamps.data_ptr()), ctypes.c_void_p(moments.data_ptr()), _stream())
+    _check(rc, "kbmod_coadd_stamps")
+    return stamps, moments
+
+
+def build_mask(sci: torch.Tensor, var: torch.Tensor, mask_in: Optional[torch.Tensor] = None, sigma_thr: float = 5.0,
+               grow: int = 2, min_images: int = 2, bright_counts: float = 120.0) -> torch.Tensor:
+    """kbmod_build_mask -> mask [N,H,W] u8."""
+    N, H, W = sci.shape
+    if var.shape != sci.shape or (mask_in is not None and mask_in.shape != sci.shape):
+        raise KbmodError("sci, var, mask_in shapes differ")
+    out = torch.empty((N, H, W), dtype=torch.uint8, device=sci.device)
+    rc = lib().kbmod_build_mask(_dev(sci, torch.float32, "sci"), _dev(var, torch.float32, "var"),
+                                _dev(mask_in, torch.uint8, "mask_in"), N, H, W, ctypes.c_float(sigma_thr), int(grow),
+                                int(min_images), ctypes.c_float(bright_counts), ctypes.c_void_p(out.data_ptr()), _stream())
+    _check(rc, "kbmod_build_mask")
+    return out

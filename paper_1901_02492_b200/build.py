@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkbmod_b200.so")
-SOURCES = ["api.cu", "psi_phi.cu", "search_direct.cu", "search_tiled.cu", "search_staged.cu"]
+SOURCES = ["api.cu", "psi_phi.cu", "search_direct.cu", "search_tiled.cu", "search_staged.cu", "postproc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC", "-Xptxas", "-v",
               "-I", os.path.join(ROOT, "include"), "-I", CSRC]

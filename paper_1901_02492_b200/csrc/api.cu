@@ -63,7 +63,7 @@ static int read_options(const kbmod_search_options* o, Options& out) {
     if (o->struct_size != 0 && o->struct_size != (int32_t)sizeof(kbmod_search_options)) return KBMOD_ERR_ARG;
     if (o->kernel < KBMOD_KERNEL_AUTO || o->kernel > KBMOD_KERNEL_TILED_QUEUED) return KBMOD_ERR_ARG;
     if (o->tile_group_w < 0 || o->tile_group_w > 256) return KBMOD_ERR_ARG;
-    if (o->staged_geom < 0 || o->staged_geom > 6) return KBMOD_ERR_ARG;
+    if (o->staged_geom < 0 || o->staged_geom > 3) return KBMOD_ERR_ARG;
     out.kernel = o->kernel;
     out.tile_group_w = o->tile_group_w;
     out.staged_geom = o->staged_geom;
@@ -237,6 +237,102 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
                  void* workspace, size_t workspace_bytes, void* stream) {
     return kbmod_search_rows(psiphi, times, N, H, W, vel_grid, V, K, min_obs, 0, H, out, workspace,
                              workspace_bytes, nullptr, stream);
+}
+
+int kbmod_search_threshold(const float* psiphi, const double* times, int N, int H, int W,
+                           const float* vel_grid, int V, int min_obs, float nu_min, int y_begin, int y_end,
+                           const kbmod_candidates* out, long long capacity, unsigned long long* count,
+                           void* workspace, size_t workspace_bytes, const kbmod_search_options* options,
+                           void* stream) {
+    if (!psiphi || !workspace || !out || !count) return KBMOD_ERR_NULL;
+    if (capacity < 0) return KBMOD_ERR_ARG;
+    if (capacity > 0 && (!out->x || !out->y || !out->vel_idx || !out->n_obs || !out->psi || !out->phi ||
+                         !out->nu || !out->alpha))
+        return KBMOD_ERR_NULL;
+    constexpr int K = 8;                                   // sizes the plan and workspace of the tiled variant
+    if (int rc = check_grid(times, N, H, W, vel_grid, V, K)) return rc;
+    if (min_obs < 1 || min_obs > N) return KBMOD_ERR_ARG;
+    if (!(nu_min == nu_min)) return KBMOD_ERR_ARG;         // NaN threshold
+    if (y_begin < 0 || y_end > H || y_begin > y_end) return KBMOD_ERR_ARG;
+    if (((uintptr_t)psiphi & 15) || ((uintptr_t)workspace & 255) || ((uintptr_t)count & 7)) return KBMOD_ERR_ALIGN;
+    const WorkspaceLayout l = workspace_layout(N, H, W, V, K);
+    if (workspace_bytes < l.total) return KBMOD_ERR_WORKSPACE;
+    Options opt;
+    if (int rc = read_options(options, opt)) return rc;
+    if (opt.kernel == KBMOD_KERNEL_TILED || opt.kernel == KBMOD_KERNEL_STAGED) return KBMOD_ERR_UNSUPPORTED;
+    DtTable dt;
+    make_dt(times, N, dt);
+    TiledPlan tplan;
+    if (opt.kernel == KBMOD_KERNEL_TILED_QUEUED)
+        if (int rc = tiled_plan_build(dt, N, H, W, vel_grid, V, K, true, tplan)) return rc;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+
+    cudaStream_t st = (cudaStream_t)stream;
+    char* ws = static_cast<char*>(workspace);
+    const float2* pp = reinterpret_cast<const float2*>(psiphi);
+    if (cudaMemsetAsync(ws + l.status_off, 0, sizeof(int), st) != cudaSuccess ||
+        cudaMemsetAsync(count, 0, sizeof(unsigned long long), st) != cudaSuccess)
+        return KBMOD_ERR_CUDA;
+    float2* vel_dev = reinterpret_cast<float2*>(ws + l.vel_off);
+    if (cudaMemcpyAsync(vel_dev, vel_grid, (size_t)V * sizeof(float2), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return KBMOD_ERR_CUDA;
+    if (opt.kernel == KBMOD_KERNEL_TILED_QUEUED)
+        return tiled_launch_threshold(tplan, pp, dt, N, H, W, min_obs, nu_min, y_begin, y_end, *out,
+                                      (unsigned long long)capacity, count, ws + l.plan_off, vel_dev,
+                                      reinterpret_cast<float2*>(ws + l.enc_off), opt.tile_group_w, st);
+    return launch_search_direct_threshold(pp, dt, N, H, W, vel_dev, V, min_obs, nu_min, y_begin, y_end, *out,
+                                          (unsigned long long)capacity, count, st);
+}
+
+int kbmod_filter_candidates(const float* psiphi, const double* times, int N, int H, int W,
+                            const int32_t* x0y0, const float* vxvy, int M, float sigma_reject,
+                            float process_var, float* psi, float* phi, int32_t* n_obs, float* nu,
+                            float* alpha, uint64_t* keep, float* kalman, void* stream) {
+    if (!psiphi || !times || !psi || !phi || !n_obs || !nu || !alpha || !keep) return KBMOD_ERR_NULL;
+    if (M > 0 && (!x0y0 || !vxvy)) return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0 || M < 0) return KBMOD_ERR_SHAPE;
+    if (N > KBMOD_MAX_IMAGES) return KBMOD_ERR_UNSUPPORTED;
+    if (!(sigma_reject > 0.0f) || !std::isfinite(sigma_reject) || !(process_var >= 0.0f) || !std::isfinite(process_var))
+        return KBMOD_ERR_ARG;
+    if (((uintptr_t)psiphi & 7) || ((uintptr_t)vxvy & 7) || ((uintptr_t)keep & 7) || ((uintptr_t)kalman & 7))
+        return KBMOD_ERR_ALIGN;
+    DtTable dt;
+    if (int rc = make_dt(times, N, dt)) return rc;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    return launch_filter_candidates(reinterpret_cast<const float2*>(psiphi), dt, N, H, W, x0y0,
+                                    reinterpret_cast<const float2*>(vxvy), M, sigma_reject, process_var, psi, phi,
+                                    n_obs, nu, alpha, reinterpret_cast<unsigned long long*>(keep),
+                                    reinterpret_cast<float2*>(kalman), (cudaStream_t)stream);
+}
+
+int kbmod_coadd_stamps(const float* sci, const uint8_t* mask, const double* times, int N, int H, int W,
+                       const int32_t* x0y0, const float* vxvy, const uint64_t* keep, int M, int R,
+                       float* stamps, float* moments, void* stream) {
+    if (!sci || !times || !stamps) return KBMOD_ERR_NULL;
+    if (M > 0 && (!x0y0 || !vxvy)) return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0 || M < 0) return KBMOD_ERR_SHAPE;
+    if (R < 0) return KBMOD_ERR_ARG;
+    if (N > KBMOD_MAX_IMAGES || R > 15) return KBMOD_ERR_UNSUPPORTED;
+    if (((uintptr_t)sci & 3) || ((uintptr_t)vxvy & 7) || ((uintptr_t)keep & 7)) return KBMOD_ERR_ALIGN;
+    DtTable dt;
+    if (int rc = make_dt(times, N, dt)) return rc;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    return launch_coadd_stamps(sci, mask, dt, N, H, W, x0y0, reinterpret_cast<const float2*>(vxvy),
+                               reinterpret_cast<const unsigned long long*>(keep), M, R, stamps, moments,
+                               (cudaStream_t)stream);
+}
+
+int kbmod_build_mask(const float* sci, const float* var, const uint8_t* mask_in, int N, int H, int W,
+                     float sigma_thr, int grow, int min_images, float bright_counts,
+                     uint8_t* mask_out, void* stream) {
+    if (!sci || !var || !mask_out) return KBMOD_ERR_NULL;
+    if (N <= 0 || H <= 0 || W <= 0) return KBMOD_ERR_SHAPE;
+    if (grow < 0 || min_images < 1 || !(sigma_thr == sigma_thr) || !(bright_counts == bright_counts)) return KBMOD_ERR_ARG;
+    if (grow > 8) return KBMOD_ERR_UNSUPPORTED;
+    if (((uintptr_t)sci & 3) || ((uintptr_t)var & 3)) return KBMOD_ERR_ALIGN;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    return launch_build_mask(sci, var, mask_in, N, H, W, sigma_thr, grow, min_images, bright_counts, mask_out,
+                             (cudaStream_t)stream);
 }
 
 int kbmod_search_status(const void* workspace, void* stream) {

@@ -8,7 +8,7 @@
 // Kernel launch.  The SIMT-emulation test build (tests/hostlogic/simt/, g++, no GPU) runs the
 // kernel's CTAs on the CPU instead; the product build is the plain triple-chevron launch.
 #if defined(KBMOD_SIMT_EMUL)
-#define KBMOD_LAUNCH(kern, grid, block, smem, stream, ...) ::simt::launch(kern, (unsigned)(grid), (unsigned)(block), (size_t)(smem), __VA_ARGS__)
+#define KBMOD_LAUNCH(kern, grid, block, smem, stream, ...) ::simt::launch(kern, ::simt::as_dim3(grid), ::simt::as_dim3(block), (size_t)(smem), __VA_ARGS__)
 #else
 #define KBMOD_LAUNCH(kern, grid, block, smem, stream, ...) kern<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__)
 #endif
@@ -30,10 +30,26 @@ int launch_psi_phi(const float* sci, const float* var, const uint8_t* mask, cons
 int launch_search_direct(const float2* psiphi, const DtTable& dt, int N, int H, int W,
                          const float2* vel_dev, int V, int K, int min_obs, int y_begin, int y_end,
                          const kbmod_result& out, cudaStream_t st);
+int launch_search_direct_threshold(const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                                   const float2* vel_dev, int V, int min_obs, float nu_min, int y_begin, int y_end,
+                                   const kbmod_candidates& out, unsigned long long capacity,
+                                   unsigned long long* count, cudaStream_t st);
 int launch_eval_trajectories(const float2* psiphi, const DtTable& dt, int N, int H, int W,
                              const int32_t* x0y0, const float2* vxvy, int M, float* Psi,
                              float* Phi, int32_t* n_obs, int32_t* ixiy, cudaStream_t st);
 int launch_interleave(const float* psi, const float* phi, size_t n, float2* out, cudaStream_t st);
+
+// ---- rows around the search (postproc.cu): N1 light-curve filter, N2 stamps + moments, N3 mask builder
+int launch_filter_candidates(const float2* psiphi, const DtTable& dt, int N, int H, int W, const int32_t* x0y0,
+                             const float2* vxvy, int M, float sigma_reject, float q, float* psi, float* phi,
+                             int32_t* n_obs, float* nu, float* alpha, unsigned long long* keep, float2* kalman,
+                             cudaStream_t st);
+int launch_coadd_stamps(const float* sci, const uint8_t* mask, const DtTable& dt, int N, int H, int W,
+                        const int32_t* x0y0, const float2* vxvy, const unsigned long long* keep, int M, int R,
+                        float* stamps, float* moments, cudaStream_t st);
+int launch_build_mask(const float* sci, const float* var, const uint8_t* mask_in, int N, int H, int W,
+                      float sigma_thr, int grow, int min_images, float bright_counts, uint8_t* mask_out,
+                      cudaStream_t st);
 
 // ---- S3: the trajectory pixel, exactly as include/kbmod_b200.h states it
 __device__ __forceinline__ bool traj_pixel(int p0, float v, float dt, int n, int& ip) {

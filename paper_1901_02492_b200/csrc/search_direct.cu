@@ -120,13 +120,54 @@ int launch_search_direct(const float2* psiphi, const DtTable& dt, int N, int H, 
     const dim3 grid((W + 31) / 32, (y_end - y_begin + 7) / 8);
     if (grid.y > 65535u) return KBMOD_ERR_UNSUPPORTED;
     if (K <= 4)
-        search_direct_kernel<4><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
+        KBMOD_LAUNCH(search_direct_kernel<4>, grid, block, 0, st, psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
     else if (K <= 8)
-        search_direct_kernel<8><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
+        KBMOD_LAUNCH(search_direct_kernel<8>, grid, block, 0, st, psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
     else if (K <= 16)
-        search_direct_kernel<16><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
+        KBMOD_LAUNCH(search_direct_kernel<16>, grid, block, 0, st, psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
     else
-        search_direct_kernel<32><<<grid, block, 0, st>>>(psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
+        KBMOD_LAUNCH(search_direct_kernel<32>, grid, block, 0, st, psiphi, dt, N, H, W, vel_dev, V, K, min_obs, y_begin, y_end, out);
+    note_launch();
+    return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
+}
+
+// N4: the paper's own retention rule ("examine those that are above a desired detection
+// threshold"): every eligible trajectory with nu >= nu_min is appended to a compacted list.
+// Same S3/S4/S5 as above; the list order is unspecified (one atomic counter), its content is not.
+__global__ void __launch_bounds__(256)
+search_direct_threshold_kernel(const float2* __restrict__ psiphi, const __grid_constant__ DtTable dt, int N,
+                               int H, int W, const float2* __restrict__ vel, int V, int min_obs, float nu_min,
+                               int y_begin, int y_end, kbmod_candidates out, unsigned long long capacity,
+                               unsigned long long* count) {
+    const int x0 = blockIdx.x * 32 + (threadIdx.x & 31);
+    const int y0 = y_begin + blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (x0 >= W || y0 >= y_end) return;
+    for (int j = 0; j < V; ++j) {
+        const float2 v = __ldg(vel + j);
+        const Coadd c = coadd_direct(psiphi, dt, N, H, W, x0, y0, v.x, v.y, nullptr);
+        if (c.n >= min_obs && c.Phi > 0.0f) {
+            const float nu = score_nu(c.Psi, c.Phi);
+            if (nu >= nu_min) {
+                const unsigned long long slot = atomicAdd(count, 1ull);
+                if (slot < capacity) {
+                    out.x[slot] = x0; out.y[slot] = y0; out.vel_idx[slot] = j; out.n_obs[slot] = c.n;
+                    out.psi[slot] = c.Psi; out.phi[slot] = c.Phi; out.nu[slot] = nu;
+                    out.alpha[slot] = score_alpha(c.Psi, c.Phi);
+                }
+            }
+        }
+    }
+}
+
+int launch_search_direct_threshold(const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                                   const float2* vel_dev, int V, int min_obs, float nu_min, int y_begin, int y_end,
+                                   const kbmod_candidates& out, unsigned long long capacity,
+                                   unsigned long long* count, cudaStream_t st) {
+    if (y_end <= y_begin) return KBMOD_OK;
+    const dim3 grid((W + 31) / 32, (y_end - y_begin + 7) / 8);
+    if (grid.y > 65535u) return KBMOD_ERR_UNSUPPORTED;
+    KBMOD_LAUNCH(search_direct_threshold_kernel, grid, 256, 0, st, psiphi, dt, N, H, W, vel_dev, V, min_obs, nu_min,
+                 y_begin, y_end, out, capacity, count);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }
@@ -150,8 +191,8 @@ int launch_eval_trajectories(const float2* psiphi, const DtTable& dt, int N, int
                              const int32_t* x0y0, const float2* vxvy, int M, float* Psi,
                              float* Phi, int32_t* n_obs, int32_t* ixiy, cudaStream_t st) {
     if (M == 0) return KBMOD_OK;
-    eval_trajectories_kernel<<<(M + 127) / 128, 128, 0, st>>>(psiphi, dt, N, H, W, x0y0, vxvy, M,
-                                                            Psi, Phi, n_obs, ixiy);
+    KBMOD_LAUNCH(eval_trajectories_kernel, (M + 127) / 128, 128, 0, st, psiphi, dt, N, H, W, x0y0, vxvy, M, Psi, Phi,
+                 n_obs, ixiy);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }
@@ -164,7 +205,7 @@ __global__ void interleave_kernel(const float* __restrict__ psi, const float* __
 }
 
 int launch_interleave(const float* psi, const float* phi, size_t n, float2* out, cudaStream_t st) {
-    interleave_kernel<<<148 * 8, 256, 0, st>>>(psi, phi, n, out);
+    KBMOD_LAUNCH(interleave_kernel, 148 * 8, 256, 0, st, psi, phi, n, out);
     note_launch();
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }

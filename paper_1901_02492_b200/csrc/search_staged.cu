@@ -50,17 +50,18 @@ static_assert(B * R == 32, "the scoring switch of search_staged_kernel lists B*R
 // ring geometry variants (samples per slot, slots); selected per call by
 // kbmod_search_options.staged_geom (tuning knob; default 0).  Smaller slots = more boxes in flight
 // but fewer windows merged per box.
-// Geometries 0-3: ring of equal slots (header + box).  Geometries 4-6: byte-granular data ring
-// (ring_alloc.h) with a separate ring of VR_NH headers, so that the boxes in flight fill the
-// whole shared memory whatever their sizes; cap = largest box.
-constexpr int NGEOM = 7;
-__host__ __device__ constexpr int cap_of(int g) {
-    return g == 0 ? 4096 : g == 1 ? 3072 : g == 2 ? 6144 : g == 3 ? 2560 : g == 4 ? 4096 : g == 5 ? 6144 : 8192;
-}
-__host__ __device__ constexpr bool is_var(int g) { return g >= 4; }
+// Geometries 0-1: ring of equal slots (header + box): 4096 samples x 6 slots, 6144 x 4.
+// Geometries 2-3: byte-granular data ring (ring_alloc.h) with a separate ring of VR_NH headers, so
+// that the boxes in flight fill the whole shared memory whatever their sizes; cap = largest box
+// (4096, 6144 samples).  The host plan's fill per sample byte at BASELINE.json configs[2] is 0.69
+// with cap 4096 and 0.68 with cap 6144; smaller caps (2560, 3072: 0.72-0.78)
+// and 8192 (0.69, fewer boxes in flight) were dropped in round 2.
+constexpr int NGEOM = 4;
+__host__ __device__ constexpr int cap_of(int g) { return (g == 0 || g == 2) ? 4096 : 6144; }
+__host__ __device__ constexpr bool is_var(int g) { return g >= 2; }
 constexpr int VR_NH = 16;                // header slots (= entries in flight at most) of the variable ring
 constexpr int VR_RING_BYTES = 212992;    // data bytes of the variable ring (208 KB)
-__host__ __device__ constexpr int nslot_of(int g) { return g == 0 ? 6 : g == 1 ? 8 : g == 2 ? 4 : g == 3 ? 10 : VR_NH; }
+__host__ __device__ constexpr int nslot_of(int g) { return g == 0 ? 6 : g == 1 ? 4 : VR_NH; }
 constexpr int HDR_INTS = 8 + 2 * B;
 constexpr int HDR_BYTES = 128;
 static_assert(HDR_INTS * 4 <= HDR_BYTES, "header");
@@ -89,9 +90,8 @@ constexpr size_t smem_bytes_of(int g) {
     return ring_bytes_of(g) + (size_t)NCW * QCAP * 12 + 2 * nslot_of(g) * 8 + VR_NH * 4;
 }
 static_assert(smem_bytes_of(0) <= 227 * 1024 && smem_bytes_of(1) <= 227 * 1024 && smem_bytes_of(2) <= 227 * 1024 &&
-              smem_bytes_of(3) <= 227 * 1024 && smem_bytes_of(4) <= 227 * 1024 && smem_bytes_of(6) <= 227 * 1024,
-              "ring does not fit shared memory");
-static_assert(cap_of(6) * 8 <= VR_RING_BYTES / 2, "a box must fit the variable ring comfortably");
+              smem_bytes_of(3) <= 227 * 1024, "ring does not fit shared memory");
+static_assert(cap_of(3) * 8 <= VR_RING_BYTES / 2, "a box must fit the variable ring comfortably");
 
 unsigned hilbert_d(unsigned x, unsigned y) {   // Hilbert index of a 16-bit quantised (x, y)
     unsigned d = 0;
@@ -875,9 +875,6 @@ static int launch_geom(int g, const StagedParams& prm, const StagedMaps& maps, i
         case 1: return launch_variant<CM, KP, 1>(prm, maps, grid, st);
         case 2: return launch_variant<CM, KP, 2>(prm, maps, grid, st);
         case 3: return launch_variant<CM, KP, 3>(prm, maps, grid, st);
-        case 4: return launch_variant<CM, KP, 4>(prm, maps, grid, st);
-        case 5: return launch_variant<CM, KP, 5>(prm, maps, grid, st);
-        case 6: return launch_variant<CM, KP, 6>(prm, maps, grid, st);
         default: return launch_variant<CM, KP, 0>(prm, maps, grid, st);
     }
 }

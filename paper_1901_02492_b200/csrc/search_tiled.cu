@@ -260,6 +260,11 @@ struct TiledParams {
     int tiles_x, tiles_y, group_w;
     kbmod_result out;
     DtTable dt;
+    // threshold mode (kbmod_search_threshold): every eligible trajectory with nu >= nu_min is appended
+    kbmod_candidates cand;
+    unsigned long long capacity;
+    unsigned long long* count;
+    float nu_min;
 };
 
 // RX x RY pixels per thread: x = tile_x + (warp % WX) * 32 * RX + rx * 32 + lane,
@@ -526,7 +531,8 @@ struct ListMemPlanes {                    // list entries are read and written t
 };
 
 // One dense pass over up to 32 queued candidates of this warp: lane l takes entry qhead + l.
-template <int RX, int KP>
+// THRESH: the candidate is appended to the compacted list if its exactly scored nu >= nu_min.
+template <int RX, int KP, bool THRESH>
 __device__ __forceinline__ void process_batch_q(const TiledParams& prm, const float* q_psi, const float* q_phi,
                                                 const unsigned* q_meta, unsigned qhead, int n, int lane,
                                                 int wx0, int wy0) {
@@ -538,6 +544,28 @@ __device__ __forceinline__ void process_batch_q(const TiledParams& prm, const fl
     const int r = pix >> 5, ln = pix & 31;
     const int x = wx0 + ln + 32 * (r % RX), y = wy0 + r / RX;
     const float nu = valid ? score_nu(Psi, Phi) : 0.0f;
+    if constexpr (THRESH) {
+        if (valid && nu >= prm.nu_min) {
+            // the sums in the queue are the in-order fp32 sums already; the literal walk adds n_obs
+            float lPsi = 0.0f, lPhi = 0.0f;
+            int cnt = 0;
+            const float2 v = __ldg(prm.vel + j);
+            for (int i = 0; i < prm.N; ++i) {
+                int ix, iy;
+                if (traj_pixel(x, v.x, prm.dt.dt[i], prm.W, ix) && traj_pixel(y, v.y, prm.dt.dt[i], prm.H, iy)) {
+                    const float2 s = __ldg(prm.psiphi + ((size_t)i * prm.H + iy) * prm.W + ix);
+                    if (s.x == s.x) { lPsi = __fadd_rn(lPsi, s.x); lPhi = __fadd_rn(lPhi, s.y); ++cnt; }
+                }
+            }
+            const unsigned long long slot = atomicAdd(prm.count, 1ull);
+            if (slot < prm.capacity) {
+                prm.cand.x[slot] = x; prm.cand.y[slot] = y; prm.cand.vel_idx[slot] = j; prm.cand.n_obs[slot] = cnt;
+                prm.cand.psi[slot] = lPsi; prm.cand.phi[slot] = lPhi; prm.cand.nu[slot] = score_nu(lPsi, lPhi);
+                prm.cand.alpha[slot] = score_alpha(lPsi, lPhi);
+            }
+        }
+        return;
+    }
     const size_t p = valid ? ((size_t)(y - prm.y_begin) * prm.W + x) * prm.K : 0;
     for (;;) {
         // two candidates of the same pixel in one batch: lowest lane first, the rest next round
@@ -556,7 +584,7 @@ __device__ __forceinline__ void process_batch_q(const TiledParams& prm, const fl
 // N <= 16): the sign bits are shifted into a history word shared by the two rx pixels of a row
 // (rx = 0 lands on the odd bits, rx = 1 on the even ones) and counted with popc when the block is
 // scored: half the counter registers, so more gathers can be in flight.
-template <int RX, int RY, int B, int KP, int CM>
+template <int RX, int RY, int B, int KP, int CM, bool THRESH = false>
 __global__ void __launch_bounds__(THREADS, 1)
 search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
     constexpr int R = RX * RY;
@@ -607,6 +635,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
 #endif
 
     // empty lists (in the output planes)
+    if constexpr (!THRESH)
 #pragma unroll
     for (int r = 0; r < R; ++r)
         if (inimg & (1u << r)) {
@@ -640,8 +669,12 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             float w = -INFINITY;
-            if (inimg & (1u << r))
-                w = __ldcg(prm.out.nu + (pix0 + 32 * (r % RX) + (size_t)(r / RX) * W) * K + (K - 1));
+            if constexpr (THRESH) {
+                w = prm.nu_min;                                  // fixed bound: the detection threshold
+            } else {
+                if (inimg & (1u << r))
+                    w = __ldcg(prm.out.nu + (pix0 + 32 * (r % RX) + (size_t)(r / RX) * W) * K + (K - 1));
+            }
             lo[r] = fmaf(-fabsf(w), 4e-6f, w);                   // -inf stays -inf
         }
 
@@ -824,7 +857,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
             }
             if (!flush) break;
             __syncwarp();
-            process_batch_q<RX, KP>(prm, q_psi, q_phi, q_meta, qhead, 32, lane, tile_x, y_first);
+            process_batch_q<RX, KP, THRESH>(prm, q_psi, q_phi, q_meta, qhead, 32, lane, tile_x, y_first);
             qhead += 32;
         }
         __syncthreads();
@@ -834,10 +867,11 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
     __syncwarp();
     while (qtail != qhead) {
         const int n = (int)min(32u, qtail - qhead);
-        process_batch_q<RX, KP>(prm, q_psi, q_phi, q_meta, qhead, n, lane, tile_x, y_first);
+        process_batch_q<RX, KP, THRESH>(prm, q_psi, q_phi, q_meta, qhead, n, lane, tile_x, y_first);
         qhead += n;
     }
     __syncwarp();
+    if constexpr (THRESH) return;                       // no per-pixel lists to finish
 #pragma unroll 1
     for (int r = 0; r < R; ++r) {
         if (!(inimg & (1u << r))) continue;
@@ -897,14 +931,14 @@ static int launch_variant(TiledParams& prm, int group_w, cudaStream_t st) {
     return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
 }
 
-template <int RX, int RY, int B, int KP, int CM>
+template <int RX, int RY, int B, int KP, int CM, bool THRESH = false>
 static int launch_variant_q(TiledParams& prm, int group_w, cudaStream_t st) {
     constexpr int TW = 32 * RX, TH = RY * (THREADS / 32);
     // two block records + the queues: 14.7 KB at N = 15, 46.8 KB at most (N = 64, B = 32), i.e. below
     // the 48 KB that need no opt-in; the rest of the SM's 256 KB stays L1 for the gathers
     const size_t smem = 2 * rec_ints(B, prm.N) * sizeof(int) + (size_t)(THREADS / 32) * QCAP * 12;
     if (smem > 48 * 1024) return KBMOD_ERR_UNSUPPORTED;
-    auto kern = search_tiledq_kernel<RX, RY, B, KP, CM>;
+    auto kern = search_tiledq_kernel<RX, RY, B, KP, CM, THRESH>;
     prm.tiles_x = (prm.W + TW - 1) / TW;
     prm.tiles_y = (prm.y_end - prm.y_begin + TH - 1) / TH;
     // tile rasterisation: groups of group_w tile columns (default 512 px wide; kbmod_search_options
@@ -939,6 +973,8 @@ int tiled_launch(const TiledPlan& plan, const float2* psiphi, const DtTable& dt,
     prm.y_begin = y_begin; prm.y_end = y_end;
     prm.out = out;
     prm.dt = dt;
+    std::memset(&prm.cand, 0, sizeof(prm.cand));
+    prm.capacity = 0; prm.count = nullptr; prm.nu_min = 0.0f;
     if (plan.queued) {                                              // kernel 4: same tiles, queue-compacted S5/S6
         const bool hist = N <= 16;                                  // history-bit counting (see CM)
         if (K <= 8) return hist ? launch_variant_q<2, 2, 8, 8, 2>(prm, group_w, st) : launch_variant_q<2, 2, 8, 8, 0>(prm, group_w, st);
@@ -948,6 +984,32 @@ int tiled_launch(const TiledPlan& plan, const float2* psiphi, const DtTable& dt,
     if (K <= 8) return launch_variant<2, 2, 1, 8, 8>(prm, group_w, st);      // tile 64 x 32
     if (K <= 16) return launch_variant<2, 1, 1, 16, 16>(prm, group_w, st);   // tile 64 x 16
     return launch_variant<1, 1, 1, 32, 32>(prm, group_w, st);                // tile 32 x 16
+}
+
+int tiled_launch_threshold(const TiledPlan& plan, const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                           int min_obs, float nu_min, int y_begin, int y_end, const kbmod_candidates& cand,
+                           unsigned long long capacity, unsigned long long* count, void* plan_dev,
+                           const float2* vel_dev, float2* enc_dev, int group_w, cudaStream_t st) {
+    if (!plan.queued) return KBMOD_ERR_ARG;
+    if (cudaMemcpyAsync(plan_dev, plan.rec.data(), plan.rec.size() * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return KBMOD_ERR_CUDA;
+    const size_t n = (size_t)N * H * W;
+    KBMOD_LAUNCH(encode_kernel, 148 * 8, 256, 0, st, reinterpret_cast<const float4*>(psiphi),
+                 reinterpret_cast<float4*>(enc_dev), n / 2, psiphi, enc_dev, n);
+    note_launch();
+    if (cudaGetLastError() != cudaSuccess) return KBMOD_ERR_CUDA;
+    TiledParams prm;
+    std::memset(&prm.out, 0, sizeof(prm.out));
+    prm.psiphi = psiphi;
+    prm.enc = reinterpret_cast<const u64*>(enc_dev);
+    prm.plan = static_cast<const int*>(plan_dev);
+    prm.vel = vel_dev;
+    prm.nblk = plan.nblk; prm.N = N; prm.H = H; prm.W = W; prm.K = 8; prm.min_obs = min_obs;   // plan blocks of 8
+    prm.y_begin = y_begin; prm.y_end = y_end;
+    prm.dt = dt;
+    prm.cand = cand; prm.capacity = capacity; prm.count = count; prm.nu_min = nu_min;
+    return N <= 16 ? launch_variant_q<2, 2, 8, 8, 2, true>(prm, group_w, st)
+                   : launch_variant_q<2, 2, 8, 8, 0, true>(prm, group_w, st);
 }
 
 int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, int W,

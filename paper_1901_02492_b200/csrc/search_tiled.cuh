@@ -32,6 +32,14 @@ int tiled_launch(const TiledPlan& plan, const float2* psiphi, const DtTable& dt,
                  int min_obs, int y_begin, int y_end, const kbmod_result& out, void* plan_dev,
                  const float2* vel_dev, float2* enc_dev, int group_w, cudaStream_t st);
 
+// Threshold mode (kbmod_search_threshold) on the queued kernel: the same gathers and pre-test with the
+// detection threshold as the bound; survivors are scored exactly and appended to the candidate list.
+// The plan must have been built with queued = true and K = 8.
+int tiled_launch_threshold(const TiledPlan& plan, const float2* psiphi, const DtTable& dt, int N, int H, int W,
+                           int min_obs, float nu_min, int y_begin, int y_end, const kbmod_candidates& cand,
+                           unsigned long long capacity, unsigned long long* count, void* plan_dev,
+                           const float2* vel_dev, float2* enc_dev, int group_w, cudaStream_t st);
+
 // plan + launch in one call
 int launch_search_tiled(const float2* psiphi, const DtTable& dt, int N, int H, int W,
                         const float* vel_host, int V, int K, int min_obs, int y_begin, int y_end,

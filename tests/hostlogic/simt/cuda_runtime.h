@@ -60,7 +60,10 @@ struct float2 { float x, y; };
 struct float4 { float x, y, z, w; };
 struct int4 { int x, y, z, w; };
 struct uint3 { unsigned x, y, z; };
-struct dim3 { unsigned x, y, z; };
+struct dim3 {
+    unsigned x, y, z;
+    dim3(unsigned x_ = 1, unsigned y_ = 1, unsigned z_ = 1) : x(x_), y(y_), z(z_) {}
+};
 static inline float2 make_float2(float x, float y) { return float2{x, y}; }
 static inline float4 make_float4(float x, float y, float z, float w) { return float4{x, y, z, w}; }
 
@@ -154,7 +157,7 @@ struct State {
     Context sched;
     Fiber* cur = nullptr;
     uint3 bid{0, 0, 0};
-    dim3 gdim{1, 1, 1}, bdim{1, 1, 1};
+    dim3 gdim, bdim;
     unsigned bar_count = 0, bar_gen = 0;
     long long steps = 0;
     unsigned rng = 1;
@@ -255,18 +258,26 @@ inline bool run_cta(unsigned nthreads, size_t smem_bytes) {
     return live == 0;
 }
 
+inline dim3 as_dim3(dim3 d) { return d; }
+inline dim3 as_dim3(unsigned v) { return dim3(v); }
+inline dim3 as_dim3(int v) { return dim3((unsigned)v); }
+inline dim3 as_dim3(long long v) { return dim3((unsigned)v); }
+
+// grids and blocks of up to two dimensions (threadIdx.x fastest, as on the device)
 template <class Kern, class... Args>
-inline void launch(Kern kern, unsigned grid, unsigned block, size_t smem_bytes, Args... args) {
+inline void launch(Kern kern, dim3 grid, dim3 block, size_t smem_bytes, Args... args) {
     State& s = S();
+    if (grid.z != 1 || block.z != 1) fatal("3-D launches are not modelled");
     ++s.launches;
-    s.gdim = dim3{grid, 1, 1};
-    s.bdim = dim3{block, 1, 1};
+    s.gdim = grid;
+    s.bdim = block;
     s.rng = cfg().seed;
-    for (unsigned b = 0; b < grid; ++b) {
-        s.bid = uint3{b, 0, 0};
-        s.body = [&]() { kern(args...); };
-        if (!run_cta(block, smem_bytes)) fatal("CTA deadlocked");
-    }
+    for (unsigned by = 0; by < grid.y; ++by)
+        for (unsigned bx = 0; bx < grid.x; ++bx) {
+            s.bid = uint3{bx, by, 0};
+            s.body = [&]() { kern(args...); };
+            if (!run_cta(block.x * block.y, smem_bytes)) fatal("CTA deadlocked");
+        }
 }
 
 // ---- shared memory access (32-bit shared-window addresses)
@@ -309,6 +320,7 @@ template <class T> static inline T __ldg(const T* p) { return *p; }
 template <class T> static inline T __ldcg(const T* p) { return *p; }
 template <class T> static inline void __stcg(T* p, T v) { *p = v; }
 static inline float __fadd_rn(float a, float b) { volatile float r = a + b; return r; }
+static inline float __fsub_rn(float a, float b) { volatile float r = a - b; return r; }
 static inline float __fmul_rn(float a, float b) { volatile float r = a * b; return r; }
 static inline float __fdiv_rn(float a, float b) { volatile float r = a / b; return r; }
 static inline float __fsqrt_rn(float a) { return sqrtf(a); }
@@ -330,6 +342,12 @@ static inline unsigned min(unsigned a, unsigned b) { return a < b ? a : b; }
 static inline int max(int a, int b) { return a > b ? a : b; }
 static inline long long clock64() { return ::simt::S().cur->clock += ::simt::cfg().clock_step; }
 static inline int atomicExch(int* p, int v) { const int o = *p; *p = v; return o; }
+// fibers never pre-empt one another inside a plain statement, so read-modify-write is atomic here
+static inline unsigned long long atomicAdd(unsigned long long* p, unsigned long long v) {
+    const unsigned long long o = *p;
+    *p = o + v;
+    return o;
+}
 
 static inline void __syncwarp(unsigned mask = ::simt::FULL) { ::simt::warp_exchange(mask, 0); }
 static inline unsigned __ballot_sync(unsigned mask, int pred) {

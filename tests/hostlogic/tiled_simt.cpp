@@ -53,6 +53,38 @@ int simt_search_tiled(const float* psiphi, const double* times, int N, int H, in
     return rc;
 }
 
+// Threshold mode on the queued kernel (kbmod_search_threshold with kernel 4).  Returns the count.
+long long simt_search_tiled_threshold(const float* psiphi, const double* times, int N, int H, int W,
+                                      const float* vel_grid, int V, int min_obs, float nu_min, int y_begin, int y_end,
+                                      long long capacity, int32_t* x, int32_t* y, int32_t* vel_idx, int32_t* n_obs,
+                                      float* psi, float* phi, float* nu, float* alpha, int order, unsigned seed) {
+    using namespace kbmod;
+    simt::cfg().order = order;
+    simt::cfg().seed = seed;
+    simt::State& s = simt::S();
+    s.smem = smem_raw;
+    s.smem_faults = s.launches = 0;
+    DtTable dt;
+    for (int i = 0; i < KBMOD_MAX_IMAGES; ++i) dt.dt[i] = 0.0f;
+    for (int i = 0; i < N; ++i) dt.dt[i] = (float)(times[i] - times[0]);
+    const size_t npix = (size_t)N * H * W, nc = (size_t)capacity * 4;
+    simt::DevBuf d_pp(psiphi, npix * 8), d_vel(vel_grid, (size_t)V * 8), d_count(8);
+    simt::DevBuf d_plan(tiled_plan_bytes(N, V, 8)), d_enc(npix * 8);
+    simt::DevBuf d_x(nc), d_y(nc), d_vi(nc), d_no(nc), d_psi(nc), d_phi(nc), d_nu(nc), d_al(nc);
+    *d_count.as<unsigned long long>() = 0;
+    kbmod_candidates out{d_x.as<int32_t>(), d_y.as<int32_t>(), d_vi.as<int32_t>(), d_no.as<int32_t>(), d_psi.as<float>(),
+                         d_phi.as<float>(), d_nu.as<float>(), d_al.as<float>()};
+    TiledPlan plan;
+    if (int rc = tiled_plan_build(dt, N, H, W, vel_grid, V, 8, true, plan)) return rc;
+    const int rc = tiled_launch_threshold(plan, d_pp.as<const float2>(), dt, N, H, W, min_obs, nu_min, y_begin, y_end, out,
+                                          (unsigned long long)capacity, d_count.as<unsigned long long>(), d_plan.p,
+                                          d_vel.as<const float2>(), d_enc.as<float2>(), 0, nullptr);
+    if (rc) return rc;
+    d_x.copy_to(x); d_y.copy_to(y); d_vi.copy_to(vel_idx); d_no.copy_to(n_obs); d_psi.copy_to(psi); d_phi.copy_to(phi);
+    d_nu.copy_to(nu); d_al.copy_to(alpha);
+    return (long long)*d_count.as<unsigned long long>();
+}
+
 // launch_search_tiled's own size limits (int16 shift encoding, int32 element offsets): the launch
 // must refuse, before touching any buffer, a stack whose (N+1)*H*W element offsets do not fit int32
 int simt_tiled_limits(int N, int H, int W, int V, int K) {

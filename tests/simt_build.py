@@ -27,13 +27,34 @@ def _stale(lib, src):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def load(name, emul_define):
-    """Compiles tests/hostlogic/<name>.cpp (which includes a csrc/*.cu file) if stale and loads it."""
+HARNESSES = {"tiled_simt": "1", "staged_simt": '"simt_ptx.h"', "post_simt": "1"}
+
+
+def build_command(name, sanitize=SANITIZE):
+    """(library path, g++ command) of tests/hostlogic/<name>.cpp (which includes csrc/*.cu files)."""
     src = os.path.join(HL, name + ".cpp")
-    lib = os.path.join(HL, f"lib{name}{'_asan' if SANITIZE else ''}.so")
-    if _stale(lib, src):
-        cmd = ["g++", "-O1", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC",
-               "-I", os.path.join(HL, "simt"), "-I", os.path.join(ROOT, "include"), "-I", CSRC,
-               f"-DKBMOD_SIMT_EMUL={emul_define}", *(SAN_FLAGS if SANITIZE else []), src, "-o", lib]
+    lib = os.path.join(HL, f"lib{name}{'_asan' if sanitize else ''}.so")
+    cmd = ["g++", "-O1", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC",
+           "-I", os.path.join(HL, "simt"), "-I", os.path.join(ROOT, "include"), "-I", CSRC,
+           f"-DKBMOD_SIMT_EMUL={HARNESSES[name]}", *(SAN_FLAGS if sanitize else []), src, "-o", lib]
+    return lib, cmd
+
+
+def build_all(sanitize=SANITIZE):
+    """Compiles every stale harness of one flavour, all at once (they are independent translation units)."""
+    procs = []
+    for name in HARNESSES:
+        lib, cmd = build_command(name, sanitize)
+        if _stale(lib, os.path.join(HL, name + ".cpp")):
+            procs.append((name, subprocess.Popen(cmd)))
+    for name, p in procs:
+        if p.wait() != 0:
+            raise RuntimeError(f"g++ failed on {name}")
+
+
+def load(name, emul_define=None):
+    """Compiles tests/hostlogic/<name>.cpp if stale and loads it."""
+    lib, cmd = build_command(name)
+    if _stale(lib, os.path.join(HL, name + ".cpp")):
         subprocess.run(cmd, check=True)
     return ctypes.CDLL(lib)

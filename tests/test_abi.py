@@ -80,7 +80,7 @@ def test_rows_options_and_plan_argument_errors(L):
                                                         ctypes.byref(opt) if opt else None, None)
     assert rows(-1, 2) == -3 and rows(3, 2) == -3 and rows(0, 5) == -3            # band outside [0, H]
     assert rows(0, 4, O(16, 9, 0, 0)) == -3 and rows(0, 4, O(16, -1, 0, 0)) == -3  # unknown kernel
-    assert rows(0, 4, O(16, 0, 300, 0)) == -3 and rows(0, 4, O(16, 3, 0, 7)) == -3 # knobs out of range
+    assert rows(0, 4, O(16, 0, 300, 0)) == -3 and rows(0, 4, O(16, 3, 0, 4)) == -3 # knobs out of range
     assert rows(0, 4, O(12, 0, 0, 0)) == -3                                         # wrong struct_size
     assert L.kbmod_search_rows(fp, t, 2, 4, 4, vel, 1, 1, 1, 0, 4, ctypes.byref(r), ws, ctypes.c_size_t(8), None, None) == -7
     # plans: host objects, no device needed

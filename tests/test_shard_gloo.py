@@ -33,7 +33,7 @@ def _worker(rank, world, port, ret):
         vel = synth.velocity_grid(4, 3, -1.0, 1.0, 2.0, 9.0)
         times = [0.0, 0.4, 1.0, 1.5]
         from tests import simt_build, test_tiled_simt as T
-        sim = simt_build.load("tiled_simt", "1")
+        sim = simt_build.load("tiled_simt")
 
         def emulated_search(psiphi, times, vel_grid, K, min_obs, y_begin, y_end):
             out = T.run_sim(sim, psiphi.numpy(), times, vel_grid, K, min_obs, T.QUEUED if rank else T.TILED,
@@ -73,7 +73,7 @@ def test_world_size_2_gloo(orc):
     ret = ctx.Manager().dict()
     port = _free_port()
     from tests import simt_build
-    simt_build.load("tiled_simt", "1")            # compile once, before the ranks race for it
+    simt_build.load("tiled_simt")            # compile once, before the ranks race for it
     procs = [ctx.Process(target=_worker, args=(r, 2, port, ret)) for r in range(2)]
     for p in procs:
         p.start()

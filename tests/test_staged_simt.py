@@ -35,7 +35,7 @@ PLANES = ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")
 
 @pytest.fixture(scope="module")
 def sim():
-    return simt_build.load("staged_simt", '"simt_ptx.h"')
+    return simt_build.load("staged_simt")
 
 
 def run_sim(sim, pp, times, vel, K, min_obs, order=0, seed=1, sms=3, tma_delay=0, geom=0, y_begin=0, y_end=None):
@@ -104,10 +104,10 @@ def test_crops_of_the_baseline_configs(sim, orc, k, over):
     assert_exact(out, ref, stats, rc)
 
 
-@pytest.mark.parametrize("geom", [1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("geom", [1, 2, 3])
 def test_ring_geometries(sim, orc, geom):
-    """Every ring geometry (kbmod_search_options.staged_geom), fixed slots (1-3) and the
-    byte-granular data ring (4-6)."""
+    """Every ring geometry (kbmod_search_options.staged_geom): fixed slots (0 is the default of the
+    other tests, 1) and the byte-granular data ring (2, 3)."""
     pp = synth.random_psiphi(9, 64, 130, seed=21, invalid_frac=0.03)
     times = np.array([0, .05, .1, .15, 1, 1.05, 1.1, 2.0, 2.05])
     vel = synth.velocity_grid(8, 6, -math.pi / 3, math.pi / 3, 3.0, 40.0)
@@ -211,10 +211,10 @@ def test_image_count_variants(sim, orc):
         assert_exact(out, ref, stats, rc)
 
 
-@pytest.mark.parametrize("geom", [0, 5])
+@pytest.mark.parametrize("geom", [0, 3])
 def test_randomized_shapes(sim, orc, geom):
     """25 seeded random problems per ring kind, random schedule, CTA count and TMA delay (a longer
-    run of the same generator, 2 025 cases on geometries 0 and 4, found no mismatch)."""
+    run of the same generator, 2 025 cases on a fixed and a variable ring, found no mismatch)."""
     from tests.test_tiled_simt import random_case
     rng = np.random.default_rng(77 + geom)
     for _ in range(25):

@@ -29,7 +29,7 @@ TILED, QUEUED = 0, 1
 
 @pytest.fixture(scope="module")
 def sim():
-    return simt_build.load("tiled_simt", '1')
+    return simt_build.load("tiled_simt")
 
 
 def run_sim(sim, pp, times, vel, K, min_obs, queued, order=0, seed=1, y_begin=0, y_end=None, group_w=0):
