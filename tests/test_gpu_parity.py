@@ -345,3 +345,52 @@ def test_search_full_size_config3_sampled_bands(kb, orc, which):
     # the injected sources are there: the best nu of the frame is far above the noise maximum (~6.5)
     best = float(res["nu"][..., 0].max().item())
     assert best > 8.0
+
+
+# ------------------------------------------------------------------------------ every BASELINE.json config at size
+def _full_size_case(kb, orc, cfg, bands):
+    """psi/phi + search at full size with the default kernel (the launch configuration bench.py
+    times); 8-row bands of start rows are recomputed by the oracle on the same psi/phi and must
+    match bit for bit; psi/phi itself is compared with the oracle on the same bands (inputs cropped
+    with the PSF halo) at the section 8(c) tolerance."""
+    kb.set_search_kernel(0)
+    st = synth.make_stack(cfg)
+    pp = kb.make_psi_phi(_cuda(st.sci), _cuda(st.var), _cuda(st.mask), st.psf)
+    res = kb.search(pp, st.times, st.vel_grid, cfg.K, cfg.min_obs)
+    r = (st.psf.shape[-1] - 1) // 2
+    for y0 in bands:
+        a, b = max(0, y0 - r), min(cfg.H, y0 + 8 + r)
+        ref_pp, pabs = orc.make_psi_phi(st.sci[:, a:b], st.var[:, a:b], st.mask[:, a:b], st.psf, want_abs=True)
+        # rows whose stencil is cut by the crop (not by the image) are not comparable: keep the band only
+        sl = slice(y0 - a, y0 - a + 8)
+        assert_psiphi_close(pp[:, y0:y0 + 8].cpu().numpy(), ref_pp[:, sl], pabs[:, sl])
+    pp_host = pp.cpu().numpy()
+    del pp
+    for y0 in bands:
+        ref = orc.search(pp_host, st.times, st.vel_grid, cfg.K, cfg.min_obs, y_begin=y0, y_end=y0 + 8)
+        gpu = {k: v[y0:y0 + 8].cpu().numpy() for k, v in res.items()}
+        assert_search_exact(gpu, ref)
+    return res
+
+
+def test_full_size_config2_ccd_night_pair(kb, orc):
+    """BASELINE.json configs[1] whole: 8 x 2048 x 4096, V = 512, K = 8, P = 19."""
+    cfg = synth.config(2)
+    res = _full_size_case(kb, orc, cfg, (0, 28, 1020, cfg.H - 8))
+    assert float(res["nu"][..., 0].max().item()) > 8.0          # the injected sources are there
+
+
+def test_full_size_config4_stress(kb, orc):
+    """BASELINE.json configs[3] whole: 12 x 4096 x 4096, V = 2048, K = 16 (64 x 16 tiles), P = 27
+    rotated elliptical PSFs (general 2-D psi/phi path), 10 % static + random masks, irregular times."""
+    cfg = synth.config(4)
+    _full_size_case(kb, orc, cfg, (0, 12, 2040, cfg.H - 8))
+
+
+@pytest.mark.parametrize("N,V", [(40, 640), (10, 8192)])
+def test_full_size_config5_sweep_corners(kb, orc, N, V):
+    """BASELINE.json configs[4], the two far corners of the sweep: the deepest stack (N = 40,
+    additive counters, 5.4 GB of psi/phi) and the largest grid (V = 8192, +-pi/2, up to 800 px/day)."""
+    na, ns = synth.SWEEP_GRIDS[V]
+    cfg = synth.config(5, N=N, n_angles=na, n_speeds=ns)
+    _full_size_case(kb, orc, cfg, (0, 2044, cfg.H - 8))
