@@ -15,6 +15,7 @@ alignas(1024) unsigned char smem_raw[simt::SMEM_MAX + 64];
 
 #include "search_direct.cu"
 #include "postproc.cu"
+#include "psi_phi.cu"
 
 namespace kbmod {
 void note_launch(int) {}
@@ -35,6 +36,23 @@ static void prep(int order, unsigned seed) {
 
 extern "C" {
 using namespace kbmod;
+
+// S1 + S2.  misalign != 0 hands the kernel a sci plane that is only 4-byte aligned, which selects the
+// scalar stage and store (round 1's path) for the same data.  launches = kernel launches issued.
+int simt_make_psi_phi(const float* sci, const float* var, const uint8_t* mask, const float* psf, int N, int H, int W,
+                      int P, float* psiphi, int misalign, int* launches, int order, unsigned seed) {
+    prep(order, seed);
+    const size_t npix = (size_t)N * H * W;
+    simt::DevBuf d_sci(npix * 4 + (misalign ? 4 : 0)), d_var(var, npix * 4), d_pp(npix * 8);
+    float* sci_dev = reinterpret_cast<float*>(d_sci.as<char>() + (misalign ? 4 : 0));
+    memcpy(sci_dev, sci, npix * 4);
+    simt::DevBuf d_mask(mask ? (const void*)mask : (const void*)sci, mask ? npix : 0);
+    const int rc = launch_psi_phi(sci_dev, d_var.as<const float>(), mask ? d_mask.as<const uint8_t>() : nullptr, psf, N, H,
+                                  W, P, d_pp.as<float2>(), nullptr);
+    d_pp.copy_to(psiphi);
+    *launches = (int)simt::S().launches;
+    return rc;
+}
 
 int simt_search_direct(const float* psiphi, const double* times, int N, int H, int W, const float* vel, int V, int K,
                        int min_obs, int y_begin, int y_end, int32_t* vel_idx, int32_t* n_obs, float* psi, float* phi,

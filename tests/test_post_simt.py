@@ -32,6 +32,62 @@ def bits_equal(a, b):
     return ((a.view(np.int32) == b.view(np.int32)) | (a == b)).all() if a.dtype == np.float32 else (a == b).all()
 
 
+# ------------------------------------------------------------------------------ S1 + S2
+def run_psi_phi(sim, sci, var, mask, psf, misalign=0):
+    N, H, W = sci.shape
+    sci, var, psf = (np.ascontiguousarray(a, np.float32) for a in (sci, var, psf))
+    out = np.zeros((N, H, W, 2), np.float32)
+    launches = ctypes.c_int(0)
+    rc = sim.simt_make_psi_phi(ptr(sci), ptr(var), ptr(mask), ptr(psf), N, H, W, psf.shape[-1], ptr(out), misalign,
+                               ctypes.byref(launches), 2, ctypes.c_uint(7))
+    assert rc == 0
+    return out, launches.value
+
+
+def assert_psiphi_close(gpu, ref, pabs):
+    gn, rn = np.isnan(gpu[..., 0]), np.isnan(ref[..., 0])
+    assert (gn == rn).all() and (gpu[..., 1][rn] == 0).all()
+    ok = ~rn
+    assert (np.abs(gpu[..., 0][ok] - ref[..., 0][ok]) <= 1e-5 * pabs[ok] + 1e-7).all()
+    assert (np.abs(gpu[..., 1][ok] - ref[..., 1][ok]) <= 1e-5 * ref[..., 1][ok] + 1e-7).all()
+
+
+@pytest.mark.parametrize("k,over", [
+    (1, {}),                                           # 64 x 64, P = 11: exactly one tile per image
+    (2, dict(N=3, H=70, W=132)),                       # several tiles + ragged tail, P = 19, W % 4 == 0
+    (4, dict(N=2, H=40, W=68, n_sources=3)),           # elliptical PSF, P = 27, 10 % static mask
+    (3, dict(N=2, H=37, W=67, n_sources=2)),           # odd width: the scalar path is the only one
+])
+def test_psi_phi_vector_and_scalar_paths(sim, orc, k, over):
+    """psi_phi_kernel in one launch for the stack: within the section 8(c) tolerance of the oracle,
+    and the float4 stage / coalesced store path bit-identical to the scalar path (round 1's)."""
+    st = synth.make_stack(synth.config(k, **over))
+    ref, pabs = orc.make_psi_phi(st.sci, st.var, st.mask, st.psf, want_abs=True)
+    vec, n_launch = run_psi_phi(sim, st.sci, st.var, st.mask, st.psf)
+    assert n_launch == 1, "the whole stack goes in one launch"
+    assert_psiphi_close(vec, ref, pabs)
+    scalar, _ = run_psi_phi(sim, st.sci, st.var, st.mask, st.psf, misalign=1)
+    assert (vec.view(np.int32) == scalar.view(np.int32)).all()
+    nomask, _ = run_psi_phi(sim, st.sci, st.var, None, st.psf)
+    ref2, pabs2 = orc.make_psi_phi(st.sci, st.var, None, st.psf, want_abs=True)
+    assert_psiphi_close(nomask, ref2, pabs2)
+
+
+def test_psi_phi_many_images_split_into_launches_and_bad_numerics(sim, orc):
+    """P = 31 takes 8 images per launch: 19 images need 3 launches; bad numerics and 1 x 1 PSFs."""
+    rng = np.random.default_rng(0)
+    sci = rng.standard_normal((19, 9, 12)).astype(np.float32)
+    var = rng.uniform(1, 2, (19, 9, 12)).astype(np.float32)
+    sci[0, 1, 1] = np.nan; sci[1, 2, 3] = np.inf; var[0, 3, 3] = 0.0; var[18, 0, 0] = -1.0; var[7, 8, 11] = np.inf
+    mask = (rng.random((19, 9, 12)) < 0.1).astype(np.uint8)
+    for P, want_launches in ((31, 3), (1, 1), (5, 1)):
+        psf = rng.uniform(0.0, 1.0, (19, P, P)).astype(np.float32)
+        ref, pabs = orc.make_psi_phi(sci, var, mask, psf, want_abs=True)
+        got, n_launch = run_psi_phi(sim, sci, var, mask, psf)
+        assert n_launch == want_launches
+        assert_psiphi_close(got, ref, pabs)
+
+
 # ------------------------------------------------------------------------------ direct search
 def run_direct(sim, pp, times, vel, K, mo, y0=0, y1=None, order=0, seed=1):
     N, H, W, _ = pp.shape
