@@ -17,6 +17,10 @@ passed the GPU suite on hardware.  The kernel and its knob
 kbmod_search_options; the host plan (kbmod_plan: it depends on times / grid / shape only) is built
 once before the timed region, as a survey pipeline searching many stacks of one cadence would.
 
+--mode threshold: the paper's own retention rule (row N4): kbmod_search_threshold with nu >= --nu-min
+(default 10) in place of the per-pixel top-K; `--config 6` is the paper's production
+grid (128 x 250 = 32 000 velocities on 13 images).  Not the driver's default workload.
+
 N > 1 (torchrun): every rank searches its own independent stack (the survey's fields/CCDs are
 independent searches) -- weak scaling, no data-path collective.  --bands (N > 1):
 ONE stack replicated on every rank, each rank searching its band of start rows through
@@ -189,7 +193,8 @@ def config_dict(cfg, args):
                         f"{cfg.H}x{cfg.W} fp32, V={cfg.V} ({cfg.n_angles}x{cfg.n_speeds}), "
                         f"K={cfg.K}, min_obs={cfg.min_obs}, seed={cfg.seed}",
             "trajectories": cfg.trajectories, "trajectory_evals": cfg.evals,
-            "step": "kbmod_make_psi_phi + kbmod_search (S1..S6)",
+            "step": ("kbmod_make_psi_phi + kbmod_search_threshold (S1..S5 + nu >= %g, row N4)" % args.nu_min
+                     if getattr(args, "mode", "topk") == "threshold" else "kbmod_make_psi_phi + kbmod_search (S1..S6)"),
             "l2": "inputs larger than L2 (stack 2.0 GB+ vs 126 MB); no flush needed",
             "parallelism": (f"one stack, start-row bands x{args.gpus} (kbmod_search_rows)" if getattr(args, "bands", False)
                             and args.gpus > 1 else f"independent stacks x{args.gpus}")}
@@ -226,17 +231,27 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     ws = torch.empty(binding.search_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
     h_out = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
     e_sci, e_var, e_mask = torch.empty_like(d_sci), torch.empty_like(d_var), torch.empty_like(d_mask)
+    h_count = torch.zeros(1, dtype=torch.int64).pin_memory()
+
+    def search_step():
+        if args.mode == "threshold":
+            return binding.search_threshold(psiphi, st.times, st.vel_grid, cfg.min_obs, args.nu_min, args.capacity,
+                                            y_begin=y0, y_end=y1, kernel=kernel, tile_group_w=args.group_w, workspace=ws)
+        return binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan, y_begin=y0, y_end=y1)
 
     def step_resident():
         binding.make_psi_phi(d_sci, d_var, d_mask, st.psf, out=psiphi)
-        binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan, y_begin=y0, y_end=y1)
+        search_step()
 
     def step_e2e():
         e_sci.copy_(h_sci, non_blocking=True)
         e_var.copy_(h_var, non_blocking=True)
         e_mask.copy_(h_mask, non_blocking=True)
         binding.make_psi_phi(e_sci, e_var, e_mask, st.psf, out=psiphi)
-        binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan, y_begin=y0, y_end=y1)
+        r = search_step()
+        if args.mode == "threshold":
+            h_count.copy_(r[0], non_blocking=True)          # the candidate list stays on the device for N1/N2
+            return
         for k in out:
             h_out[k].copy_(out[k], non_blocking=True)
 
@@ -282,8 +297,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
         return float(np.median(ts))
     reps = max(3, min(args.steps, 10))
     ms_psiphi = phase(lambda: binding.make_psi_phi(d_sci, d_var, d_mask, st.psf, out=psiphi), reps)
-    ms_search = phase(lambda: binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws,
-                                             plan=plan, y_begin=y0, y_end=y1), reps)
+    ms_search = phase(search_step, reps)
 
     binding.search_status(ws)
     step_e2e()
@@ -294,8 +308,8 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     # reported beside `e2e`, and only if its result planes equal the resident run's
     host_abi = None
     try:
-        if world > 1:
-            raise RuntimeError("measured at N=1 only")
+        if world > 1 or args.mode == "threshold":
+            raise RuntimeError("measured at N=1 in top-K mode only")
         ws_h = torch.empty(binding.search_host_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
         run_h = lambda: binding.search_host(h_sci, h_var, h_mask, st.psf, st.times, st.vel_grid, K,
                                             cfg.min_obs, h_out, ws_h, kernel=kernel)
@@ -330,7 +344,8 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     # equal to the resident run's; the same step driven from Python (torch pinned-memory copies
     # around kbmod_make_psi_phi + kbmod_search) is reported beside it and is the fallback.
     xfer = {"h2d_bytes_per_step": int(h_sci.numel() * 4 + h_var.numel() * 4 + h_mask.numel()),
-            "d2h_bytes_per_step": int(sum(v.numel() * v.element_size() for v in h_out.values()))}
+            "d2h_bytes_per_step": (8 if args.mode == "threshold" else
+                                   int(sum(v.numel() * v.element_size() for v in h_out.values())))}
     e2e_binding = {"value": evals / (e2e_ms / e2e_steps * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / e2e_steps,
                    "path": "torch pinned H2D copies + kbmod_make_psi_phi + kbmod_search + torch D2H copies", **xfer}
     if host_abi and "value" in host_abi and world == 1:
@@ -394,6 +409,10 @@ def main():
                          "3 TMA-staged, 4 tiled + queued top-K (3 and 4: opt-in, see DESIGN.md section 8)")
     ap.add_argument("--group-w", type=int, default=0, help="kbmod_search_options.tile_group_w (0 = default)")
     ap.add_argument("--staged-geom", type=int, default=0, help="kbmod_search_options.staged_geom (kernel 3)")
+    ap.add_argument("--mode", default="topk", choices=["topk", "threshold"],
+                    help="topk: kbmod_search (BASELINE.json's metric); threshold: kbmod_search_threshold (row N4)")
+    ap.add_argument("--nu-min", type=float, default=10.0, help="--mode threshold: detection threshold (PAPER.md:237)")
+    ap.add_argument("--capacity", type=int, default=1 << 24, help="--mode threshold: candidate list capacity")
     ap.add_argument("--bands", action="store_true",
                     help="N > 1: one replicated stack, one band of start rows per rank (strong scaling)")
     ap.add_argument("--ref-rows", type=int, default=256, help="start rows per oracle sample")

@@ -80,7 +80,10 @@ class StackConfig:
 
 def config(k: int, **over) -> StackConfig:
     """BASELINE.json configs[k-1] (k = 1..5).  Config 5 is a sweep: pass N=..., and
-    n_angles/n_speeds for the grid point (defaults: N=10, 32x20)."""
+    n_angles/n_speeds for the grid point (defaults: N=10, 32x20).  k = 6 is not a BASELINE.json
+    config: it is the paper's own production search (13 images over three nights,
+    128 angles within +-12 degrees x 250 speeds over 1-5.7 arcsec/hour = 92.3-526 px/day at 0.26
+    arcsec/px, 32 000 velocities per start pixel, threshold nu >= 10), the workload of row N4."""
     if k == 1:
         c = StackConfig(
             name="c1_tiny", N=5, H=64, W=64, seed=1,
@@ -115,6 +118,14 @@ def config(k: int, **over) -> StackConfig:
             n_sources=100, flux_lo=100.0, flux_hi=2000.0,
             n_angles=32, n_speeds=20, ang_lo=-math.pi / 2, ang_hi=math.pi / 2,
             speed_lo=50.0, speed_hi=800.0, K=8, min_obs=(N + 1) // 2)
+    elif k == 6:
+        c = StackConfig(
+            name="c6_hits_production", N=13, H=4096, W=4096, seed=6,
+            epochs_per_night=5, epoch_spacing=0.0625,                  # 5 + 5 + 3 epochs over three nights
+            var_lo=80.0, var_hi=150.0, sigma_lo=1.2, sigma_hi=1.8, mask_frac=0.01,
+            n_sources=200, flux_lo=100.0, flux_hi=2000.0,
+            n_angles=128, n_speeds=250, ang_lo=-math.radians(12.0), ang_hi=math.radians(12.0),
+            speed_lo=24.0 / 0.26, speed_hi=5.7 * 24.0 / 0.26, K=8, min_obs=7)
     else:
         raise ValueError(f"no config {k}")
     return replace(c, **over) if over else c

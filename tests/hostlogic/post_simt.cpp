@@ -70,6 +70,19 @@ int simt_search_direct(const float* psiphi, const double* times, int N, int H, i
     return rc;
 }
 
+int simt_eval_trajectories(const float* psiphi, const double* times, int N, int H, int W, const int32_t* x0y0,
+                           const float* vxvy, int M, float* Psi, float* Phi, int32_t* n_obs, int32_t* ixiy) {
+    prep(0, 1);
+    simt::DevBuf d_pp(psiphi, (size_t)N * H * W * 8), d_xy(x0y0, (size_t)M * 8), d_v(vxvy, (size_t)M * 8);
+    simt::DevBuf d_psi((size_t)M * 4), d_phi((size_t)M * 4), d_no((size_t)M * 4), d_ix((size_t)M * N * 8);
+    const int rc = launch_eval_trajectories(d_pp.as<const float2>(), dt_of(times, N), N, H, W, d_xy.as<const int32_t>(),
+                                            d_v.as<const float2>(), M, d_psi.as<float>(), d_phi.as<float>(),
+                                            d_no.as<int32_t>(), ixiy ? d_ix.as<int32_t>() : nullptr, nullptr);
+    d_psi.copy_to(Psi); d_phi.copy_to(Phi); d_no.copy_to(n_obs);
+    if (ixiy) d_ix.copy_to(ixiy);
+    return rc;
+}
+
 long long simt_search_direct_threshold(const float* psiphi, const double* times, int N, int H, int W, const float* vel,
                                        int V, int min_obs, float nu_min, int y_begin, int y_end, long long capacity,
                                        int32_t* x, int32_t* y, int32_t* vel_idx, int32_t* n_obs, float* psi, float* phi,

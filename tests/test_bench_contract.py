@@ -60,6 +60,12 @@ def stubbed(monkeypatch):
     def search_host(*a, kernel=None):
         calls["launches"] += 3
 
+    def search_threshold(*a, **k):
+        calls["launches"] += 1
+        calls["threshold"] = calls.get("threshold", 0) + 1
+        return torch.zeros(1, dtype=torch.int64), {}
+
+    b.search_threshold = search_threshold
     b.make_psi_phi, b.search, b.search_host = make_psi_phi, search, search_host
     b.search_status = lambda ws: None
     b.launch_count = lambda: calls["launches"]
@@ -130,6 +136,14 @@ def test_explicit_kernel_goes_into_the_options(stubbed, monkeypatch):
     assert stubbed["kernel"] == [4] and d["search_options"] == {**d["search_options"], "kernel": 4, "tile_group_w": 4}
     assert "search_tiledq_kernel" in d["search_kernel"]
     assert "cpu_baseline" not in d
+
+
+def test_threshold_mode_line(stubbed, monkeypatch):
+    """Row N4 as a bench workload: the step is psi/phi + kbmod_search_threshold; only the count
+    comes back to the host."""
+    d = run_main(monkeypatch, ["--config", "1", "--steps", "2", "--mode", "threshold", "--nu-min", "7", "--no-cpu"])
+    assert stubbed["threshold"] >= 2 + 3 and "kbmod_search_threshold" in d["config"]["step"]
+    assert d["e2e"]["d2h_bytes_per_step"] == 8 and d["gpu_launches"] == 4
 
 
 def test_reference_arm_line(monkeypatch):

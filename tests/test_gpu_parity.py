@@ -15,6 +15,8 @@ import torch
 
 from paper_1901_02492_b200 import synth
 
+# KBMOD_GPU_TESTS_EMULATED=1: run this file's LOGIC against the SIMT-emulated library on CPU tensors
+EMULATED = os.environ.get("KBMOD_GPU_TESTS_EMULATED") == "1"
 pytestmark = pytest.mark.gpu
 
 # 1 = direct gather, 0 = automatic (the tiled kernel where the shape fits), 3 = TMA-staged kernel.
@@ -25,16 +27,20 @@ KERNELS = [1, 0] + ([3] if os.environ.get("KBMOD_TEST_STAGED") == "1" else [])
 
 @pytest.fixture(scope="module")
 def kb():
-    from paper_1901_02492_b200 import binding
-    if not torch.cuda.is_available():
-        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    if EMULATED:                     # test-logic check on a machine without a GPU (tests/emulated_binding.py)
+        from tests import emulated_binding as binding
+    else:
+        from paper_1901_02492_b200 import binding
+        if not torch.cuda.is_available():
+            pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
     binding.lib()
     yield binding
     binding.set_search_kernel(0)
 
 
 def _cuda(a):
-    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    return t if EMULATED else t.cuda()
 
 
 def _np(res):

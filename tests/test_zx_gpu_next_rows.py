@@ -14,21 +14,27 @@ import torch
 
 from paper_1901_02492_b200 import synth
 
+# KBMOD_GPU_TESTS_EMULATED=1: run this file's LOGIC against the SIMT-emulated library on CPU tensors
+EMULATED = os.environ.get("KBMOD_GPU_TESTS_EMULATED") == "1"
 pytestmark = pytest.mark.gpu
 CAND = ("x", "y", "vel_idx", "n_obs", "psi", "phi", "nu", "alpha")
 
 
 @pytest.fixture(scope="module")
 def kb():
-    from paper_1901_02492_b200 import binding
-    if not torch.cuda.is_available():
-        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    if EMULATED:                     # test-logic check on a machine without a GPU (tests/emulated_binding.py)
+        from tests import emulated_binding as binding
+    else:
+        from paper_1901_02492_b200 import binding
+        if not torch.cuda.is_available():
+            pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
     binding.lib()
     return binding
 
 
 def _cuda(a):
-    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    return t if EMULATED else t.cuda()
 
 
 def _bits(a, b):
@@ -105,7 +111,7 @@ def test_search_then_filter_removes_an_interloper(kb, orc):
     flat = torch.topk(nu.flatten(), 200).indices
     ys, xs = (flat // cfg.W).int(), (flat % cfg.W).int()
     x0y0 = torch.stack([xs, ys], 1).contiguous()
-    vel = torch.from_numpy(st.vel_grid).cuda()[res["vel_idx"][..., 0].flatten()[flat].long()].contiguous()
+    vel = _cuda(st.vel_grid)[res["vel_idx"][..., 0].flatten()[flat].long()].contiguous()
     out = kb.filter_candidates(pp, st.times, x0y0, vel)
     ref = orc.filter_candidates(pp.cpu().numpy(), st.times, x0y0.cpu().numpy(), vel.cpu().numpy())
     assert (out["keep"].cpu().numpy().view(np.uint64) == ref["keep"]).all()

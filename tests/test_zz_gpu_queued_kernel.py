@@ -17,6 +17,8 @@ from tests import test_gpu_parity as P
 # Opt-in (KBMOD_TEST_QUEUED=1), exactly like kernel 3 behind KBMOD_TEST_STAGED: a kernel enters the
 # default GPU suite only after this file has passed on hardware in the builder's own run (the kept
 # output is under profiles/).
+# KBMOD_GPU_TESTS_EMULATED=1: run this file's LOGIC against the SIMT-emulated library on CPU tensors
+EMULATED = os.environ.get("KBMOD_GPU_TESTS_EMULATED") == "1"
 pytestmark = [pytest.mark.gpu,
               pytest.mark.skipif(os.environ.get("KBMOD_TEST_QUEUED") != "1",
                                  reason="kernel 4 is opt-in: set KBMOD_TEST_QUEUED=1")]
@@ -25,9 +27,12 @@ QUEUED = 4
 
 @pytest.fixture(scope="module")
 def kb():
-    from paper_1901_02492_b200 import binding
-    if not torch.cuda.is_available():
-        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    if EMULATED:                     # test-logic check on a machine without a GPU (tests/emulated_binding.py)
+        from tests import emulated_binding as binding
+    else:
+        from paper_1901_02492_b200 import binding
+        if not torch.cuda.is_available():
+            pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
     binding.lib()
     yield binding
     binding.set_search_kernel(0)
