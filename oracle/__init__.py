@@ -242,3 +242,19 @@ def coadd_stamps(sci, mask, times, x0y0, vxvy, keep=None, R=10):
     if rc != 0:
         raise ValueError(f"oracle_coadd_stamps failed: {rc}")
     return stamps, moments
+
+
+def cluster_candidates(x0y0, vxvy, nu, eps_xy=2.0, eps_v=4.0, min_samples=1):
+    """N5 -> label [M] i32 (smallest core index of the cluster, -1 = noise), rep [M] u8."""
+    x0y0 = _c(x0y0, np.int32).reshape(-1, 2)
+    vxvy = _c(vxvy, np.float32).reshape(-1, 2)
+    nu = _c(nu, np.float32)
+    M = x0y0.shape[0]
+    label = np.zeros(M, np.int32)
+    rep = np.zeros(M, np.uint8)
+    lib().oracle_cluster_candidates.restype = ctypes.c_int
+    rc = lib().oracle_cluster_candidates(_p(x0y0), _p(vxvy), _p(nu), M, ctypes.c_float(eps_xy), ctypes.c_float(eps_v),
+                                         int(min_samples), _p(label), _p(rep))
+    if rc != 0:
+        raise ValueError(f"oracle_cluster_candidates failed: {rc}")
+    return label, rep

@@ -635,3 +635,78 @@ int oracle_coadd_stamps(const float* sci, const uint8_t* mask, const double* tim
     free(dt);
     return ORACLE_OK;
 }
+
+/*
+ * N5. De-duplication of candidates by DBSCAN.  P:249 (section 3.3): "We take the starting x and y
+ * pixels and the horizontal and vertical velocities of the candidate trajectories and use the DBSCAN
+ * clustering method (Ester et al. 1996) ... to group similar trajectories.  We then take the highest
+ * likelihood trajectory for each group".  eps and min_samples are not given (PARITY UNPINNED against
+ * the paper); reading N5-a..N5-c of DESIGN.md:
+ *   neighbours   a, b are neighbours iff d2 <= 1 with
+ *                d2 = fl( fl(fl(dx*dx + dy*dy) * ixy) + fl(fl(fl(dvx*dvx) + fl(dvy*dvy)) * iv) ),
+ *                dx, dy exact integers, dvx = fl(vx_a - vx_b), ixy = fl(1/fl(eps_xy^2)), iv = fl(1/fl(eps_v^2));
+ *                every point is its own neighbour;
+ *   DBSCAN       core iff it has >= min_samples neighbours; clusters = connected components of the core
+ *                points; label = smallest index of a core point of the component (canonical, unique);
+ *                a non-core point with core neighbours takes the smallest label among them (DBSCAN
+ *                leaves this choice open); without any it is noise, label -1;
+ *   keep         rep = 1 for the member of each cluster with the largest nu (ties: smaller index) and
+ *                for every noise point.
+ */
+static int cl_neighbours(const int32_t* xy, const float* v, int a, int b, float ixy, float iv) {
+    const long long dx = (long long)xy[2 * a] - xy[2 * b], dy = (long long)xy[2 * a + 1] - xy[2 * b + 1];
+    volatile float r2 = (float)(dx * dx + dy * dy);
+    volatile float dvx = v[2 * a] - v[2 * b], dvy = v[2 * a + 1] - v[2 * b + 1];
+    volatile float sx = dvx * dvx, sy = dvy * dvy;
+    volatile float v2 = sx + sy;
+    volatile float ta = r2 * ixy, tb = v2 * iv;
+    volatile float d2 = ta + tb;
+    return d2 <= 1.0f;
+}
+
+int oracle_cluster_candidates(const int32_t* x0y0, const float* vxvy, const float* nu, int M, float eps_xy,
+                              float eps_v, int min_samples, int32_t* label, uint8_t* rep) {
+    if (M < 0 || (M > 0 && (!x0y0 || !vxvy || !nu || !label || !rep))) return ORACLE_ERR_ARG;
+    if (!(eps_xy > 0.0f) || !(eps_v > 0.0f) || min_samples < 1) return ORACLE_ERR_ARG;
+    volatile float exy2 = eps_xy * eps_xy, ev2 = eps_v * eps_v;
+    volatile float ixy = 1.0f / exy2, iv = 1.0f / ev2;
+    uint8_t* core = (uint8_t*)calloc(M ? M : 1, 1);
+    for (int i = 0; i < M; ++i) {
+        int n = 0;
+        for (int j = 0; j < M; ++j) n += cl_neighbours(x0y0, vxvy, i, j, ixy, iv);
+        core[i] = n >= min_samples;
+        label[i] = -1;
+    }
+    int* stack = (int*)malloc(sizeof(int) * (M ? M : 1));
+    for (int s = 0; s < M; ++s) {                       /* components in order of their smallest core index */
+        if (!core[s] || label[s] >= 0) continue;
+        int top = 0;
+        stack[top++] = s;
+        label[s] = s;
+        while (top) {
+            const int i = stack[--top];
+            for (int j = 0; j < M; ++j)
+                if (core[j] && label[j] < 0 && cl_neighbours(x0y0, vxvy, i, j, ixy, iv)) {
+                    label[j] = s;
+                    stack[top++] = j;
+                }
+        }
+    }
+    for (int i = 0; i < M; ++i) {
+        if (core[i]) continue;
+        int best = -1;
+        for (int j = 0; j < M; ++j)
+            if (core[j] && cl_neighbours(x0y0, vxvy, i, j, ixy, iv) && (best < 0 || label[j] < best)) best = label[j];
+        label[i] = best;
+    }
+    for (int i = 0; i < M; ++i) {
+        int r = 1;
+        if (label[i] >= 0)
+            for (int j = 0; j < M && r; ++j)
+                if (j != i && label[j] == label[i] && (nu[j] > nu[i] || (nu[j] == nu[i] && j < i))) r = 0;
+        rep[i] = (uint8_t)r;
+    }
+    free(stack);
+    free(core);
+    return ORACLE_OK;
+}

@@ -254,3 +254,56 @@ def test_n2_central_moments_against_float64_numpy(orc):
     # an empty stamp: all zero
     _, mo = orc.coadd_stamps(np.zeros((1, 9, 9), np.float32), None, [0.0], [[4, 4]], [[0.0, 0.0]], None, 2)
     assert (mo == 0).all()
+
+
+# ------------------------------------------------------------------------------------------ N5
+@pytest.mark.parametrize("min_samples", [1, 3])
+def test_n5_clusters_against_sklearn_dbscan(orc, min_samples):
+    """scikit-learn's DBSCAN (the routine the paper used) on the scaled 4-D points: same core
+    points, same partition of the core points, same noise; border points (whose cluster DBSCAN leaves
+    open) must sit in a cluster with one of their core neighbours.  Coordinates on a coarse lattice,
+    so no distance is within rounding of eps."""
+    from sklearn.cluster import DBSCAN
+    rng = np.random.default_rng(50 + min_samples)
+    centres = np.stack([rng.integers(0, 400, 40), rng.integers(0, 400, 40),
+                        rng.integers(-40, 40, 40) * 4, rng.integers(-40, 40, 40) * 4], 1)
+    pts = np.concatenate([centres[rng.integers(0, 40, 500)] +
+                          np.stack([rng.integers(-2, 3, 500), rng.integers(-2, 3, 500),
+                                    rng.integers(-2, 3, 500) * 2, rng.integers(-2, 3, 500) * 2], 1),
+                          np.stack([rng.integers(0, 400, 60), rng.integers(0, 400, 60),
+                                    rng.integers(-160, 160, 60), rng.integers(-160, 160, 60)], 1)])
+    x0y0, vxvy = pts[:, :2].astype(np.int32), pts[:, 2:].astype(np.float32)
+    nu = rng.uniform(5, 50, len(pts)).astype(np.float32)
+    eps_xy, eps_v = 2.5, 4.5
+    label, rep = orc.cluster_candidates(x0y0, vxvy, nu, eps_xy, eps_v, min_samples)
+    X = np.concatenate([x0y0 / eps_xy, vxvy.astype(np.float64) / eps_v], 1)
+    ref = DBSCAN(eps=1.0, min_samples=min_samples).fit(X)
+    core = np.zeros(len(pts), bool)
+    core[ref.core_sample_indices_] = True
+    assert ((label == -1) == (ref.labels_ == -1)).all()
+    # same partition of the core points: a bijection between the two labelings
+    pairs = set(zip(label[core], ref.labels_[core]))
+    assert len(pairs) == len(set(label[core])) == len(set(ref.labels_[core]))
+    # canonical label = smallest core index of the cluster
+    for lab in set(label[core]):
+        assert lab == np.flatnonzero(core & (label == lab)).min()
+    d2 = ((X[:, None, :] - X[None, :, :]) ** 2).sum(-1)
+    for i in np.flatnonzero(~core & (label >= 0)):            # border points
+        nb = np.flatnonzero(core & (d2[i] <= 1.0))
+        assert len(nb) and label[i] == label[nb].min()
+    # one representative per cluster: its brightest member; every noise point is kept
+    for lab in set(label[label >= 0]):
+        mem = np.flatnonzero(label == lab)
+        assert rep[mem].sum() == 1 and nu[mem[rep[mem] == 1][0]] == nu[mem].max()
+    assert rep[label == -1].all()
+    if min_samples == 3:
+        assert (label == -1).any() and (~core & (label >= 0)).any(), "the case must contain noise and border points"
+
+
+def test_n5_degenerate_inputs(orc):
+    label, rep = orc.cluster_candidates(np.zeros((0, 2), np.int32), np.zeros((0, 2), np.float32), np.zeros(0, np.float32))
+    assert len(label) == 0 and len(rep) == 0
+    xy = np.array([[5, 5], [5, 5], [5, 6], [100, 100]], np.int32)
+    v = np.zeros((4, 2), np.float32)
+    label, rep = orc.cluster_candidates(xy, v, np.array([3.0, 3.0, 1.0, 9.0], np.float32), 1.5, 1.0, 1)
+    assert list(label) == [0, 0, 0, 3] and list(rep) == [1, 0, 0, 1]       # equal nu: the smaller index wins
