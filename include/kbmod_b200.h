@@ -12,7 +12,7 @@
  * Conventions
  *   - Plain C, no torch / C++ types.  Pointers are DEVICE pointers unless marked HOST.
  *   - The library never allocates or frees caller-visible memory and never synchronises the
- *     stream.  The caller (PyTorch in this repo) owns every buffer and the stream.  HOST
+ *     stream (two documented exceptions: kbmod_search_status and kbmod_cluster_candidates).  The caller (PyTorch in this repo) owns every buffer and the stream.  HOST
  *     arrays are consumed before the call returns.
  *   - Images are row-major [N][H][W], x (column) fastest.  Integer coordinates are pixel
  *     centres; pixel ix covers [ix-0.5, ix+0.5).
@@ -256,6 +256,27 @@ int kbmod_coadd_stamps(const float* sci, const uint8_t* mask, const double* time
 int kbmod_build_mask(const float* sci, const float* var, const uint8_t* mask_in, int N, int H, int W,
                      float sigma_thr, int grow, int min_images, float bright_counts,
                      uint8_t* mask_out, void* stream);
+
+/*
+ * De-duplication of candidates (section 3.3: DBSCAN over the start pixel and the velocity,
+ * "the highest likelihood trajectory for each group").  eps and min_samples are not given in the
+ * paper; reading DESIGN.md N5-a..N5-c: candidates a, b are neighbours iff
+ *     (dx^2 + dy^2)/eps_xy^2 + (dvx^2 + dvy^2)/eps_v^2 <= 1        (fp32, fixed operation order);
+ * a candidate is a core point iff it has >= min_samples neighbours (itself included); clusters are
+ * the connected components of the core points, labelled by their smallest core index; a non-core
+ * candidate with core neighbours takes the smallest label among them, without any it is noise
+ * (label -1).  rep = 1 for the member of largest nu of each cluster (ties: smaller index) and for
+ * every noise candidate.
+ *   x0y0 : [M][2] int32 device;  vxvy : [M][2] float device (8-byte aligned);  nu : [M] float device
+ *   label : [M] int32 device;  rep : [M] uint8 device
+ *   workspace : device scratch of kbmod_cluster_workspace(M) bytes, 256-byte aligned
+ * All-pairs passes (O(M^2)): meant for the 1e2..1e5 candidates that survive the filters.
+ * This call SYNCHRONISES the stream (label propagation runs until nothing changes).
+ */
+int kbmod_cluster_candidates(const int32_t* x0y0, const float* vxvy, const float* nu, int M,
+                             float eps_xy, float eps_v, int min_samples, int32_t* label, uint8_t* rep,
+                             void* workspace, size_t workspace_bytes, void* stream);
+size_t kbmod_cluster_workspace(int M);
 
 /* Completion status of the last kbmod_search that used this workspace.  SYNCHRONISES the stream
  * (the one call of the library that does).  KBMOD_OK, or KBMOD_ERR_TIMEOUT if a warp of the

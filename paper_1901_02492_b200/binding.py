@@ -22,8 +22,8 @@ EXPORTS = ("kbmod_make_psi_phi", "kbmod_search", "kbmod_search_rows", "kbmod_sea
            "kbmod_plan_destroy", "kbmod_eval_trajectories", "kbmod_launch_count", "kbmod_status_string",
            "kbmod_version", "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host",
            "kbmod_search_host_workspace", "kbmod_search_threshold", "kbmod_filter_candidates",
-           "kbmod_coadd_stamps", "kbmod_build_mask")
-_INT_CALLS = ("kbmod_search_threshold", "kbmod_filter_candidates", "kbmod_coadd_stamps", "kbmod_build_mask",
+           "kbmod_coadd_stamps", "kbmod_build_mask", "kbmod_cluster_candidates", "kbmod_cluster_workspace")
+_INT_CALLS = ("kbmod_cluster_candidates", "kbmod_search_threshold", "kbmod_filter_candidates", "kbmod_coadd_stamps", "kbmod_build_mask",
               "kbmod_make_psi_phi", "kbmod_search", "kbmod_search_rows", "kbmod_search_split",
               "kbmod_plan_create", "kbmod_plan_kernel", "kbmod_search_planned", "kbmod_eval_trajectories",
               "kbmod_debug_staged_plan", "kbmod_search_status", "kbmod_search_host")
@@ -66,6 +66,7 @@ def lib() -> ctypes.CDLL:
         L = ctypes.CDLL(LIB_PATH)
         L.kbmod_search_workspace.restype = ctypes.c_size_t
         L.kbmod_search_host_workspace.restype = ctypes.c_size_t
+        L.kbmod_cluster_workspace.restype = ctypes.c_size_t
         L.kbmod_launch_count.restype = ctypes.c_ulonglong
         L.kbmod_status_string.restype = ctypes.c_char_p
         L.kbmod_version.restype = ctypes.c_char_p
@@ -448,3 +449,21 @@ def build_mask(sci: torch.Tensor, var: torch.Tensor, mask_in: Optional[torch.Ten
                                 int(min_images), ctypes.c_float(bright_counts), ctypes.c_void_p(out.data_ptr()), _stream())
     _check(rc, "kbmod_build_mask")
     return out
+
+
+def cluster_candidates(x0y0: torch.Tensor, vxvy: torch.Tensor, nu: torch.Tensor, eps_xy: float = 2.0,
+                       eps_v: float = 4.0, min_samples: int = 1):
+    """kbmod_cluster_candidates -> label [M] i32 (-1 = noise), rep [M] u8.  Synchronises the stream."""
+    M = int(x0y0.shape[0])
+    if tuple(x0y0.shape) != (M, 2) or tuple(vxvy.shape) != (M, 2) or tuple(nu.shape) != (M,):
+        raise KbmodError("x0y0, vxvy must be [M,2], nu [M]")
+    dev = x0y0.device
+    label = torch.empty(M, dtype=torch.int32, device=dev)
+    rep = torch.empty(M, dtype=torch.uint8, device=dev)
+    ws = torch.empty(int(lib().kbmod_cluster_workspace(M)), dtype=torch.uint8, device=dev)
+    rc = lib().kbmod_cluster_candidates(_dev(x0y0, torch.int32, "x0y0"), _dev(vxvy, torch.float32, "vxvy"),
+                                        _dev(nu, torch.float32, "nu"), M, ctypes.c_float(eps_xy), ctypes.c_float(eps_v),
+                                        int(min_samples), ctypes.c_void_p(label.data_ptr()), ctypes.c_void_p(rep.data_ptr()),
+                                        _dev(ws, torch.uint8, "workspace"), ctypes.c_size_t(ws.numel()), _stream())
+    _check(rc, "kbmod_cluster_candidates")
+    return label, rep

@@ -335,6 +335,22 @@ int kbmod_build_mask(const float* sci, const float* var, const uint8_t* mask_in,
                              (cudaStream_t)stream);
 }
 
+size_t kbmod_cluster_workspace(int M) { return M < 0 ? 0 : cluster_workspace_bytes(M); }
+
+int kbmod_cluster_candidates(const int32_t* x0y0, const float* vxvy, const float* nu, int M,
+                             float eps_xy, float eps_v, int min_samples, int32_t* label, uint8_t* rep,
+                             void* workspace, size_t workspace_bytes, void* stream) {
+    if (M < 0) return KBMOD_ERR_SHAPE;
+    if (M > 0 && (!x0y0 || !vxvy || !nu || !label || !rep || !workspace)) return KBMOD_ERR_NULL;
+    if (!(eps_xy > 0.0f) || !(eps_v > 0.0f) || !std::isfinite(eps_xy) || !std::isfinite(eps_v) || min_samples < 1)
+        return KBMOD_ERR_ARG;
+    if (((uintptr_t)vxvy & 7) || ((uintptr_t)workspace & 255)) return KBMOD_ERR_ALIGN;
+    if (M > 0 && workspace_bytes < cluster_workspace_bytes(M)) return KBMOD_ERR_WORKSPACE;
+    if (!have_device()) return KBMOD_ERR_CUDA;
+    return launch_cluster_candidates(x0y0, reinterpret_cast<const float2*>(vxvy), nu, M, eps_xy, eps_v, min_samples,
+                                     label, rep, workspace, (cudaStream_t)stream);
+}
+
 int kbmod_search_status(const void* workspace, void* stream) {
     if (!workspace) return KBMOD_ERR_NULL;
     if ((uintptr_t)workspace & 255) return KBMOD_ERR_ALIGN;

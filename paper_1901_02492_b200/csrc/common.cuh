@@ -51,6 +51,11 @@ int launch_build_mask(const float* sci, const float* var, const uint8_t* mask_in
                       float sigma_thr, int grow, int min_images, float bright_counts, uint8_t* mask_out,
                       cudaStream_t st);
 
+size_t cluster_workspace_bytes(int M);
+int launch_cluster_candidates(const int32_t* x0y0, const float2* vxvy, const float* nu, int M, float eps_xy,
+                              float eps_v, int min_samples, int32_t* label, uint8_t* rep, void* workspace,
+                              cudaStream_t st);
+
 // ---- S3: the trajectory pixel, exactly as include/kbmod_b200.h states it
 __device__ __forceinline__ bool traj_pixel(int p0, float v, float dt, int n, int& ip) {
     const float f = __fadd_rn(__int2float_rn(p0), __fmul_rn(v, dt));

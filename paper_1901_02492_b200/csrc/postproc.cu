@@ -267,3 +267,150 @@ int launch_build_mask(const float* sci, const float* var, const uint8_t* mask_in
 }
 
 }  // namespace kbmod
+
+// ---------------------------------------------------------------------------------------------
+// N5  (section 3.3): DBSCAN over (x0, y0, vx, vy), brightest member per cluster
+// ---------------------------------------------------------------------------------------------
+// Candidate lists are short (the paper's filters leave 1e2..1e5 per field), so all-pairs passes are
+// the simple and regular choice: every kernel below walks the M points in shared-memory tiles.
+// The neighbour test is the fixed binary32 sequence DESIGN.md N5-a states; labels are canonical
+// (smallest core index of the component), found by min-label propagation with pointer jumping.
+namespace kbmod {
+
+constexpr int CL_THREADS = 256;
+constexpr int CL_NOLABEL = 0x7FFFFFFF;
+
+struct ClPoint { int x, y; float vx, vy; };
+
+__device__ __forceinline__ bool cl_neighbours(const ClPoint& a, const ClPoint& b, float ixy, float iv) {
+    const long long dx = (long long)a.x - b.x, dy = (long long)a.y - b.y;
+    const float r2 = (float)(dx * dx + dy * dy);
+    const float dvx = __fsub_rn(a.vx, b.vx), dvy = __fsub_rn(a.vy, b.vy);
+    const float v2 = __fadd_rn(__fmul_rn(dvx, dvx), __fmul_rn(dvy, dvy));
+    return __fadd_rn(__fmul_rn(r2, ixy), __fmul_rn(v2, iv)) <= 1.0f;
+}
+
+__device__ __forceinline__ ClPoint cl_load(const int32_t* x0y0, const float2* vxvy, int i) {
+    const float2 v = vxvy[i];
+    return ClPoint{x0y0[2 * i], x0y0[2 * i + 1], v.x, v.y};
+}
+
+// mode 0: core[i] = (#neighbours >= min_samples), label[i] = core ? i : NOLABEL
+// mode 1: one propagation step over core points: label[i] = min(label[i], labels of core neighbours); *changed |= moved
+// mode 2: border / noise: non-core i takes the smallest label among its core neighbours, else -1
+// mode 3: rep[i] = no member of the same cluster ranks before i (larger nu; equal nu: smaller index); noise: 1
+__global__ void __launch_bounds__(CL_THREADS)
+cluster_pass_kernel(int mode, const int32_t* __restrict__ x0y0, const float2* __restrict__ vxvy,
+                    const float* __restrict__ nu, int M, float ixy, float iv, int min_samples, uint8_t* core,
+                    const int32_t* label_in, int32_t* label_out, uint8_t* rep, int* changed) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    ClPoint* s_pt = reinterpret_cast<ClPoint*>(smem_raw);                       // [CL_THREADS]
+    int* s_lab = reinterpret_cast<int*>(s_pt + CL_THREADS);                     // label (or core flag in mode 0)
+    float* s_nu = reinterpret_cast<float*>(s_lab + CL_THREADS);
+    unsigned char* s_core = reinterpret_cast<unsigned char*>(s_nu + CL_THREADS);
+    const int i = blockIdx.x * CL_THREADS + threadIdx.x;
+    const bool live = i < M;
+    const ClPoint me = live ? cl_load(x0y0, vxvy, i) : ClPoint{0, 0, 0.0f, 0.0f};
+    const int my_lab = (live && mode != 0) ? label_in[i] : CL_NOLABEL;
+    const bool my_core = (live && mode != 0) ? core[i] != 0 : false;
+    const float my_nu = (live && mode == 3) ? nu[i] : 0.0f;
+    int count = 0, best = CL_NOLABEL;
+    bool beaten = false;
+    for (int j0 = 0; j0 < M; j0 += CL_THREADS) {
+        __syncthreads();
+        const int j = j0 + threadIdx.x;
+        if (j < M) {
+            s_pt[threadIdx.x] = cl_load(x0y0, vxvy, j);
+            s_lab[threadIdx.x] = mode != 0 ? label_in[j] : 0;
+            s_core[threadIdx.x] = mode != 0 ? core[j] : 0;
+            s_nu[threadIdx.x] = mode == 3 ? nu[j] : 0.0f;
+        }
+        __syncthreads();
+        const int n = min(CL_THREADS, M - j0);
+        if (!live) continue;
+        for (int k = 0; k < n; ++k) {
+            if (mode == 3) {
+                if (my_lab >= 0 && s_lab[k] == my_lab && j0 + k != i &&
+                    (s_nu[k] > my_nu || (s_nu[k] == my_nu && j0 + k < i)))
+                    beaten = true;
+                continue;
+            }
+            if (mode != 0 && !s_core[k]) continue;
+            if (!cl_neighbours(me, s_pt[k], ixy, iv)) continue;
+            ++count;
+            best = min(best, s_lab[k]);
+        }
+    }
+    if (!live) return;
+    if (mode == 0) {
+        const bool c = count >= min_samples;
+        core[i] = c;
+        label_out[i] = c ? i : CL_NOLABEL;
+    } else if (mode == 1) {
+        int l = my_lab;
+        if (my_core && best < l) { l = best; *changed = 1; }
+        label_out[i] = l;
+    } else if (mode == 2) {
+        label_out[i] = my_core ? my_lab : (best == CL_NOLABEL ? -1 : best);
+    } else {
+        rep[i] = (my_lab < 0 || !beaten) ? 1 : 0;
+    }
+}
+
+// pointer jumping between propagation steps: a core point's label is a core index of its own
+// component (or its own), so label[label[i]] is a smaller-or-equal index of the same component
+__global__ void __launch_bounds__(CL_THREADS)
+cluster_jump_kernel(const uint8_t* __restrict__ core, const int32_t* label_in, int32_t* label_out, int M) {
+    const int i = blockIdx.x * CL_THREADS + threadIdx.x;
+    if (i >= M) return;
+    int l = label_in[i];
+    if (core[i]) {
+        const int l2 = label_in[l];
+        if (l2 < l) l = l2;
+    }
+    label_out[i] = l;
+}
+
+size_t cluster_workspace_bytes(int M) {
+    const size_t m = (size_t)(M > 0 ? M : 1);
+    return ((m + 255) / 256 * 256) + 2 * ((m * 4 + 255) / 256 * 256) + 256;      // core, two label buffers, flag
+}
+
+// SYNCHRONISES the stream once per propagation round (the number of rounds depends on the data).
+int launch_cluster_candidates(const int32_t* x0y0, const float2* vxvy, const float* nu, int M, float eps_xy,
+                              float eps_v, int min_samples, int32_t* label, uint8_t* rep, void* workspace,
+                              cudaStream_t st) {
+    if (M == 0) return KBMOD_OK;
+    volatile float exy2 = eps_xy * eps_xy, ev2 = eps_v * eps_v;
+    volatile float ixy = 1.0f / exy2, iv = 1.0f / ev2;
+    char* ws = static_cast<char*>(workspace);
+    const size_t mb = ((size_t)M + 255) / 256 * 256, lb = ((size_t)M * 4 + 255) / 256 * 256;
+    uint8_t* core = reinterpret_cast<uint8_t*>(ws);
+    int32_t* la = reinterpret_cast<int32_t*>(ws + mb);
+    int32_t* lb_ = reinterpret_cast<int32_t*>(ws + mb + lb);
+    int* flag = reinterpret_cast<int*>(ws + mb + 2 * lb);
+    const unsigned grid = (unsigned)((M + CL_THREADS - 1) / CL_THREADS);
+    const size_t smem = CL_THREADS * (sizeof(ClPoint) + 4 + 4 + 1);
+    auto pass = [&](int mode, const int32_t* lin, int32_t* lout) {
+        KBMOD_LAUNCH(cluster_pass_kernel, grid, CL_THREADS, smem, st, mode, x0y0, vxvy, nu, M, (float)ixy, (float)iv,
+                     min_samples, core, lin, lout, rep, flag);
+        note_launch();
+    };
+    pass(0, nullptr, la);
+    for (int round = 0; round < M + 1; ++round) {
+        if (cudaMemsetAsync(flag, 0, sizeof(int), st) != cudaSuccess) return KBMOD_ERR_CUDA;
+        pass(1, la, lb_);
+        KBMOD_LAUNCH(cluster_jump_kernel, grid, CL_THREADS, 0, st, core, lb_, la, M);
+        note_launch();
+        int changed = 0;
+        if (cudaMemcpyAsync(&changed, flag, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess)
+            return KBMOD_ERR_CUDA;
+        if (!changed) break;
+    }
+    pass(2, la, label);
+    pass(3, label, nullptr);
+    return cudaGetLastError() == cudaSuccess ? KBMOD_OK : KBMOD_ERR_CUDA;
+}
+
+}  // namespace kbmod

@@ -218,3 +218,14 @@ def build_mask(sci, var, mask_in=None, sigma_thr=5.0, grow=2, min_images=2, brig
     if rc:
         raise KbmodError(f"kbmod_build_mask failed: {rc}")
     return torch.from_numpy(out)
+
+
+def cluster_candidates(x0y0, vxvy, nu, eps_xy=2.0, eps_v=4.0, min_samples=1):
+    xy, v, n_ = _np(x0y0, np.int32), _np(vxvy, np.float32), _np(nu, np.float32)
+    M = xy.shape[0]
+    label, rep, n = np.zeros(M, np.int32), np.zeros(M, np.uint8), ctypes.c_int(0)
+    rc = _lib("post_simt").simt_cluster_candidates(_p(xy), _p(v), _p(n_), M, ctypes.c_float(eps_xy), ctypes.c_float(eps_v),
+                                                   int(min_samples), _p(label), _p(rep), ctypes.byref(n), 2, ctypes.c_uint(1))
+    if rc:
+        raise KbmodError(f"kbmod_cluster_candidates failed: {rc}")
+    return torch.from_numpy(label), torch.from_numpy(rep)

@@ -136,6 +136,19 @@ int simt_coadd_stamps(const float* sci, const uint8_t* mask, const double* times
     return rc;
 }
 
+int simt_cluster_candidates(const int32_t* x0y0, const float* vxvy, const float* nu, int M, float eps_xy, float eps_v,
+                            int min_samples, int32_t* label, uint8_t* rep, int* launches, int order, unsigned seed) {
+    prep(order, seed);
+    simt::DevBuf d_xy(x0y0, (size_t)M * 8), d_v(vxvy, (size_t)M * 8), d_nu(nu, (size_t)M * 4);
+    simt::DevBuf d_lab((size_t)M * 4), d_rep((size_t)M), d_ws(cluster_workspace_bytes(M));
+    const int rc = launch_cluster_candidates(d_xy.as<const int32_t>(), d_v.as<const float2>(), d_nu.as<const float>(), M,
+                                             eps_xy, eps_v, min_samples, d_lab.as<int32_t>(), d_rep.as<uint8_t>(), d_ws.p,
+                                             nullptr);
+    d_lab.copy_to(label); d_rep.copy_to(rep);
+    *launches = (int)simt::S().launches;
+    return rc;
+}
+
 int simt_build_mask(const float* sci, const float* var, const uint8_t* mask_in, int N, int H, int W, float sigma_thr,
                     int grow, int min_images, float bright, uint8_t* mask_out, int order, unsigned seed) {
     prep(order, seed);

@@ -268,3 +268,34 @@ def test_build_mask_matches_the_oracle_exactly(sim, orc):
                                      ctypes.c_float(120.0), ptr(got), 1, ctypes.c_uint(1))
             assert rc == 0 and (got == want).all()
             assert want.any() and (H < 10 or not want.all())
+
+
+# ------------------------------------------------------------------------------ N5
+def test_cluster_candidates_matches_the_oracle_exactly(sim, orc):
+    """DBSCAN by min-label propagation + pointer jumping: same canonical labels and representatives
+    as the oracle's flood fill, incl. chains (many propagation rounds), border points, noise, ties."""
+    rng = np.random.default_rng(61)
+    cases = []
+    centres = np.stack([rng.integers(0, 300, 30), rng.integers(0, 300, 30), rng.integers(-30, 30, 30) * 4,
+                        rng.integers(-30, 30, 30) * 4], 1)
+    pts = np.concatenate([centres[rng.integers(0, 30, 600)] +
+                          np.stack([rng.integers(-2, 3, 600), rng.integers(-2, 3, 600), rng.integers(-2, 3, 600) * 2,
+                                    rng.integers(-2, 3, 600) * 2], 1),
+                          np.stack([rng.integers(0, 300, 70), rng.integers(0, 300, 70), rng.integers(-120, 120, 70),
+                                    rng.integers(-120, 120, 70)], 1)])
+    cases.append((pts, 2.5, 4.5))
+    chain = np.stack([np.arange(700)[::-1] * 2, np.zeros(700, int), np.zeros(700, int), np.zeros(700, int)], 1)   # one long chain
+    cases.append((chain, 2.0, 1.0))
+    cases.append((np.array([[5, 5, 0, 0]]), 1.0, 1.0))
+    for pts, exy, ev in cases:
+        x0y0, vxvy = np.ascontiguousarray(pts[:, :2], np.int32), np.ascontiguousarray(pts[:, 2:], np.float32)
+        M = len(pts)
+        nu = np.round(rng.uniform(5, 50, M)).astype(np.float32)             # rounded: exact ties occur
+        for ms in (1, 3):
+            want_l, want_r = orc.cluster_candidates(x0y0, vxvy, nu, exy, ev, ms)
+            label, rep, n = np.zeros(M, np.int32), np.zeros(M, np.uint8), ctypes.c_int(0)
+            rc = sim.simt_cluster_candidates(ptr(x0y0), ptr(vxvy), ptr(nu), M, ctypes.c_float(exy), ctypes.c_float(ev), ms,
+                                             ptr(label), ptr(rep), ctypes.byref(n), 2, ctypes.c_uint(ms))
+            assert rc == 0 and (label == want_l).all() and (rep == want_r).all()
+        if M == 700:
+            assert n.value < 60, "pointer jumping: a chain of 700 must not need 700 rounds"

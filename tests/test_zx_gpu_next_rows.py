@@ -1,6 +1,6 @@
 """GPU parity of the rows around the search, through the C ABI against the
 CPU oracle on the same seeded inputs: N4 threshold-mode search, N1 light-curve filter, N2 coadded
-stamps and moments, N3 mask builder.  Bars: every integer / bit-mask / index output bit-exact; every
+stamps and moments, N3 mask builder, N5 DBSCAN de-duplication.  Bars: every integer / bit-mask / index output bit-exact; every
 float bit-exact too (each is a fixed sequence of separately rounded binary32 operations that the
 oracle restates).  The device logic of these kernels is checked on the CPU first
 (tests/test_post_simt.py, also under AddressSanitizer); this file sorts after tests/test_gpu_parity.py.
@@ -163,3 +163,38 @@ def test_build_mask_matches_oracle_and_feeds_psi_phi(kb, orc):
     psf = synth.gaussian_psf_kernels([1.2] * N, [1.2] * N, [0.0] * N, 7)
     pp = kb.make_psi_phi(_cuda(sci), _cuda(var), got, psf).cpu().numpy()
     assert (np.isnan(pp[..., 0]) == (want != 0) | ~np.isfinite(sci) | ~(var > 0)).all()
+
+
+def test_cluster_candidates_matches_oracle(kb, orc):
+    """N5 on the device: canonical DBSCAN labels and representatives equal the oracle's, and the
+    whole chain search -> threshold list -> de-duplication collapses the near-duplicates around the
+    injected source of config 1 and keeps its brightest trajectory."""
+    rng = np.random.default_rng(61)
+    centres = np.stack([rng.integers(0, 300, 30), rng.integers(0, 300, 30), rng.integers(-30, 30, 30) * 4,
+                        rng.integers(-30, 30, 30) * 4], 1)
+    pts = np.concatenate([centres[rng.integers(0, 30, 3000)] +
+                          np.stack([rng.integers(-2, 3, 3000), rng.integers(-2, 3, 3000), rng.integers(-2, 3, 3000) * 2,
+                                    rng.integers(-2, 3, 3000) * 2], 1),
+                          np.stack([rng.integers(0, 300, 200), rng.integers(0, 300, 200), rng.integers(-120, 120, 200),
+                                    rng.integers(-120, 120, 200)], 1),
+                          np.stack([np.arange(900)[::-1] * 2 + 1000, np.zeros(900, int), np.zeros(900, int),
+                                    np.zeros(900, int)], 1)])
+    x0y0, vxvy = np.ascontiguousarray(pts[:, :2], np.int32), np.ascontiguousarray(pts[:, 2:], np.float32)
+    nu = np.round(rng.uniform(5, 50, len(pts))).astype(np.float32)
+    for ms in (1, 3):
+        want_l, want_r = orc.cluster_candidates(x0y0, vxvy, nu, 2.5, 4.5, ms)
+        label, rep = kb.cluster_candidates(_cuda(x0y0), _cuda(vxvy), _cuda(nu), 2.5, 4.5, ms)
+        assert (label.cpu().numpy() == want_l).all() and (rep.cpu().numpy() == want_r).all()
+    cfg = synth.config(1)
+    st = synth.make_stack(cfg)
+    pp = kb.make_psi_phi(_cuda(st.sci), _cuda(st.var), _cuda(st.mask), st.psf)
+    count, got = kb.search_threshold(pp, st.times, st.vel_grid, cfg.min_obs, 12.0, 4096)
+    n = int(count.item())
+    assert 2 <= n <= 4096
+    xy = torch.stack([got["x"][:n], got["y"][:n]], 1).contiguous()
+    vel = _cuda(st.vel_grid)[got["vel_idx"][:n].long()].contiguous()
+    label, rep = kb.cluster_candidates(xy, vel, got["nu"][:n].contiguous(), 3.0, 8.0, 1)
+    keep = rep.cpu().numpy() == 1
+    assert 1 <= keep.sum() <= n // 8          # hundreds of near-duplicates collapse to a handful of groups
+    b = int(torch.argmax(got["nu"][:n]).item())
+    assert keep[b] and abs(int(got["x"][b]) - 20) <= 1 and abs(int(got["y"][b]) - 30) <= 1
