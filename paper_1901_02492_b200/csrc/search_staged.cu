@@ -33,6 +33,7 @@
 #include <cuda.h>
 
 #include "ring_alloc.h"
+#include "search_common.cuh"
 #include "search_staged.cuh"
 #include "topk_list.h"
 
@@ -92,19 +93,6 @@ constexpr size_t smem_bytes_of(int g) {
 static_assert(smem_bytes_of(0) <= 227 * 1024 && smem_bytes_of(1) <= 227 * 1024 && smem_bytes_of(2) <= 227 * 1024 &&
               smem_bytes_of(3) <= 227 * 1024, "ring does not fit shared memory");
 static_assert(cap_of(3) * 8 <= VR_RING_BYTES / 2, "a box must fit the variable ring comfortably");
-
-unsigned hilbert_d(unsigned x, unsigned y) {   // Hilbert index of a 16-bit quantised (x, y)
-    unsigned d = 0;
-    for (unsigned s = 1u << 15; s > 0; s >>= 1) {
-        const unsigned rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
-        d += s * s * ((3u * rx) ^ ry);
-        if (ry == 0) {
-            if (rx == 1) { x = 65535u - x; y = 65535u - y; }
-            std::swap(x, y);
-        }
-    }
-    return d;
-}
 
 // The literal S3 of include/kbmod_b200.h on the host (IEEE binary32, no contraction possible:
 // two dependent additions).  d = fl(v*dt) is formed by the caller.
@@ -167,20 +155,7 @@ inline bool box_fits(int bw, int bh, int cap) { return bw <= MAXBW && bh <= 256 
 // Builds the entry stream.  Returns false when the box shapes cannot be brought under MAXMAPS.
 static bool build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, int cap, StagedPlan& plan) {
     plan.nent = 0;
-    // processing order: Hilbert curve over the velocity plane (ties: index)
-    float lox = vel[0], hix = vel[0], loy = vel[1], hiy = vel[1];
-    for (int j = 1; j < V; ++j) {
-        lox = std::min(lox, vel[2 * j]); hix = std::max(hix, vel[2 * j]);
-        loy = std::min(loy, vel[2 * j + 1]); hiy = std::max(hiy, vel[2 * j + 1]);
-    }
-    const double ext = std::max({(double)hix - lox, (double)hiy - loy, 1e-30});
-    std::vector<std::pair<unsigned, int>> key(V);
-    for (int j = 0; j < V; ++j) {
-        const unsigned qx = (unsigned)std::min(65535.0, ((double)vel[2 * j] - lox) / ext * 65535.0);
-        const unsigned qy = (unsigned)std::min(65535.0, ((double)vel[2 * j + 1] - loy) / ext * 65535.0);
-        key[j] = {hilbert_d(qx, qy), j};
-    }
-    std::sort(key.begin(), key.end());
+    const std::vector<std::pair<unsigned, int>> key = hilbert_order(vel, V);    // processing order
 
     // proven shifts, per (velocity, image): 0 = skip (no observation possible), 1 = proven, 2 = unsafe
     std::vector<unsigned char> kind((size_t)V * N);
@@ -752,45 +727,13 @@ search_staged_kernel(const __grid_constant__ StagedParams prm, const __grid_cons
                 for (;;) {
                     bool flush = false;
                     switch (step) {
-#define KBMOD_SCORE_STEP(S)                                                                              \
-    case S: {                                                                                            \
-        constexpr int b_ = (S) / R, r_ = (S) % R;                                                        \
-        const int j = lds32(sa + 32 + 4 * B + 4 * b_);                                                   \
-        if (j >= 0) {                                                                                    \
-            const float Psi = __uint_as_float((unsigned)acc[b_][r_]);                                    \
-            const float Phi = 0.0f - __uint_as_float((unsigned)(acc[b_][r_] >> 32));                     \
-            unsigned n;                                                                                  \
-            if constexpr (CM == 2) n = __popc(cnt[b_][r_ / RX] & ((r_ % RX) ? 0x55555555u : 0xAAAAAAAAu)); \
-            else if constexpr (CM == 1) n = __popc(cnt[b_][r_ % NC]);                                    \
-            else n = cnt[b_][r_ % NC];                                                                   \
-            const bool pass = (n >= minobs) && (Phi > 0.0f) && ((inimg >> r_) & 1u) &&                   \
-                              !(Psi * rsqrtf(Phi) < lo[r_]);                                             \
-            const unsigned m = __ballot_sync(0xFFFFFFFFu, pass);                                         \
-            if (m) {                                                                                     \
-                if (pass) {                                                                              \
-                    const unsigned qi = (qtail + __popc(m & ((1u << lane) - 1u))) & (QCAP - 1);          \
-                    sts32(qb + 4 * qi, __float_as_int(Psi));                                             \
-                    sts32(qb + 4 * QCAP + 4 * qi, __float_as_int(Phi));                                  \
-                    sts32(qb + 8 * QCAP + 4 * qi, (j << 7) | (r_ << 5) | lane);                          \
-                }                                                                                        \
-                qtail += __popc(m);                                                                      \
-                if (qtail - qhead >= 32) {                                                               \
-                    step = (S) + 1;                                                                      \
-                    flush = true;                                                                        \
-                    break;                                                                               \
-                }                                                                                        \
-            }                                                                                            \
-        }                                                                                                \
-    }
-                        KBMOD_SCORE_STEP(0) KBMOD_SCORE_STEP(1) KBMOD_SCORE_STEP(2) KBMOD_SCORE_STEP(3)
-                        KBMOD_SCORE_STEP(4) KBMOD_SCORE_STEP(5) KBMOD_SCORE_STEP(6) KBMOD_SCORE_STEP(7)
-                        KBMOD_SCORE_STEP(8) KBMOD_SCORE_STEP(9) KBMOD_SCORE_STEP(10) KBMOD_SCORE_STEP(11)
-                        KBMOD_SCORE_STEP(12) KBMOD_SCORE_STEP(13) KBMOD_SCORE_STEP(14) KBMOD_SCORE_STEP(15)
-                        KBMOD_SCORE_STEP(16) KBMOD_SCORE_STEP(17) KBMOD_SCORE_STEP(18) KBMOD_SCORE_STEP(19)
-                        KBMOD_SCORE_STEP(20) KBMOD_SCORE_STEP(21) KBMOD_SCORE_STEP(22) KBMOD_SCORE_STEP(23)
-                        KBMOD_SCORE_STEP(24) KBMOD_SCORE_STEP(25) KBMOD_SCORE_STEP(26) KBMOD_SCORE_STEP(27)
-                        KBMOD_SCORE_STEP(28) KBMOD_SCORE_STEP(29) KBMOD_SCORE_STEP(30) KBMOD_SCORE_STEP(31)
-#undef KBMOD_SCORE_STEP
+#define KBMOD_VEL_OF(b) lds32(sa + 32 + 4 * B + 4 * (b))
+#define KBMOD_QPUT(qi, Psi, Phi, meta)                                                       \
+    (sts32(qb + 4 * (qi), __float_as_int(Psi)), sts32(qb + 4 * QCAP + 4 * (qi), __float_as_int(Phi)), \
+     sts32(qb + 8 * QCAP + 4 * (qi), (int)(meta)))
+                        KBMOD_SCORE_STEPS_32(KBMOD_VEL_OF, KBMOD_QPUT)
+#undef KBMOD_VEL_OF
+#undef KBMOD_QPUT
                         default: break;
                     }
                     if (!flush) break;

@@ -28,6 +28,7 @@
 #include <cstring>
 #include <vector>
 
+#include "search_common.cuh"
 #include "search_tiled.cuh"
 #include "topk_list.h"
 
@@ -50,20 +51,6 @@ constexpr int META = 8;                   // ints of per-velocity meta data in a
 __host__ __device__ inline size_t rec_ints(int B, int N) { return (size_t)B * N * 2 + (size_t)B * META; }
 
 int block_size_for_k(int K) { return K <= 8 ? 8 : (K <= 16 ? 16 : 32); }
-
-// ---- Hilbert index of a 16-bit quantised (x, y)
-unsigned hilbert_d(unsigned x, unsigned y) {
-    unsigned d = 0;
-    for (unsigned s = 1u << 15; s > 0; s >>= 1) {
-        const unsigned rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
-        d += s * s * ((3u * rx) ^ ry);
-        if (ry == 0) {
-            if (rx == 1) { x = 65535u - x; y = 65535u - y; }
-            std::swap(x, y);
-        }
-    }
-    return d;
-}
 
 }  // namespace
 
@@ -96,20 +83,7 @@ int tiled_plan_build(const DtTable& dt, int N, int H, int W, const float* vel_ho
 // depend on the order in which velocities are visited.
 static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, int B,
                       std::vector<int>& plan, bool isolate) {
-    // processing order: Hilbert curve over the velocity plane (ties and order of equal keys: index)
-    float lox = vel[0], hix = vel[0], loy = vel[1], hiy = vel[1];
-    for (int j = 1; j < V; ++j) {
-        lox = std::min(lox, vel[2 * j]); hix = std::max(hix, vel[2 * j]);
-        loy = std::min(loy, vel[2 * j + 1]); hiy = std::max(hiy, vel[2 * j + 1]);
-    }
-    const double ext = std::max({(double)hix - lox, (double)hiy - loy, 1e-30});
-    std::vector<std::pair<unsigned, int>> key(V);
-    for (int j = 0; j < V; ++j) {
-        const unsigned qx = (unsigned)std::min(65535.0, ((double)vel[2 * j] - lox) / ext * 65535.0);
-        const unsigned qy = (unsigned)std::min(65535.0, ((double)vel[2 * j + 1] - loy) / ext * 65535.0);
-        key[j] = {hilbert_d(qx, qy), j};
-    }
-    std::sort(key.begin(), key.end());
+    const std::vector<std::pair<unsigned, int>> key = hilbert_order(vel, V);    // processing order
 
     // largest coordinate magnitude any fl(x0 + d) can reach for an in-range window
     const double cmax = 2.0 * std::max(W, H) + 4.0;
@@ -815,44 +789,11 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
         for (;;) {
             bool flush = false;
             switch (step) {
-#define KBMOD_SCORE_STEP(S)                                                                              \
-    case S: {                                                                                            \
-        constexpr int b_ = (S) / R, r_ = (S) % R;                                                        \
-        const int j = r_meta[b_ * META + 0];                                                             \
-        if (j >= 0) {                                                                                    \
-            const float Psi = __uint_as_float((unsigned)acc[b_][r_]);                                    \
-            const float Phi = 0.0f - __uint_as_float((unsigned)(acc[b_][r_] >> 32));                     \
-            unsigned n;                                                                                  \
-            if constexpr (CM == 2) n = __popc(cnt[b_][r_ / RX] & ((r_ % RX) ? 0x55555555u : 0xAAAAAAAAu)); \
-            else n = cnt[b_][r_ % NC];                                                                   \
-            const bool pass = (n >= minobs) && (Phi > 0.0f) && ((inimg >> r_) & 1u) &&                   \
-                              !(Psi * rsqrtf(Phi) < lo[r_]);                                             \
-            const unsigned m = __ballot_sync(0xFFFFFFFFu, pass);                                         \
-            if (m) {                                                                                     \
-                if (pass) {                                                                              \
-                    const unsigned qi = (qtail + __popc(m & ((1u << lane) - 1u))) & (QCAP - 1);          \
-                    q_psi[qi] = Psi;                                                                     \
-                    q_phi[qi] = Phi;                                                                     \
-                    q_meta[qi] = ((unsigned)j << 7) | (r_ << 5) | lane;                                  \
-                }                                                                                        \
-                qtail += __popc(m);                                                                      \
-                if (qtail - qhead >= 32) {                                                               \
-                    step = (S) + 1;                                                                      \
-                    flush = true;                                                                        \
-                    break;                                                                               \
-                }                                                                                        \
-            }                                                                                            \
-        }                                                                                                \
-    }
-                KBMOD_SCORE_STEP(0) KBMOD_SCORE_STEP(1) KBMOD_SCORE_STEP(2) KBMOD_SCORE_STEP(3)
-                KBMOD_SCORE_STEP(4) KBMOD_SCORE_STEP(5) KBMOD_SCORE_STEP(6) KBMOD_SCORE_STEP(7)
-                KBMOD_SCORE_STEP(8) KBMOD_SCORE_STEP(9) KBMOD_SCORE_STEP(10) KBMOD_SCORE_STEP(11)
-                KBMOD_SCORE_STEP(12) KBMOD_SCORE_STEP(13) KBMOD_SCORE_STEP(14) KBMOD_SCORE_STEP(15)
-                KBMOD_SCORE_STEP(16) KBMOD_SCORE_STEP(17) KBMOD_SCORE_STEP(18) KBMOD_SCORE_STEP(19)
-                KBMOD_SCORE_STEP(20) KBMOD_SCORE_STEP(21) KBMOD_SCORE_STEP(22) KBMOD_SCORE_STEP(23)
-                KBMOD_SCORE_STEP(24) KBMOD_SCORE_STEP(25) KBMOD_SCORE_STEP(26) KBMOD_SCORE_STEP(27)
-                KBMOD_SCORE_STEP(28) KBMOD_SCORE_STEP(29) KBMOD_SCORE_STEP(30) KBMOD_SCORE_STEP(31)
-#undef KBMOD_SCORE_STEP
+#define KBMOD_VEL_OF(b) r_meta[(b) * META + 0]
+#define KBMOD_QPUT(qi, Psi, Phi, meta) (q_psi[qi] = (Psi), q_phi[qi] = (Phi), q_meta[qi] = (meta))
+                KBMOD_SCORE_STEPS_32(KBMOD_VEL_OF, KBMOD_QPUT)
+#undef KBMOD_VEL_OF
+#undef KBMOD_QPUT
                 default: break;
             }
             if (!flush) break;
