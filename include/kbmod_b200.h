@@ -142,6 +142,7 @@ int kbmod_search(const float* psiphi, const double* times, int N, int H, int W,
  * of one replicated stack searched on different GPUs concatenate to the full search (row-band
  * sharding).  Trajectories still sample the whole images.
  *   out       : planes of the BAND only, each [(y_end - y_begin)][W][K]; row 0 = start row y_begin
+ *               (an empty band, y_begin == y_end, writes nothing and accepts NULL planes)
  *   options   : HOST, may be NULL
  * Other arguments as kbmod_search (the workspace size does not depend on the band).
  */

@@ -82,9 +82,11 @@ static int check_grid(const double* times, int N, int H, int W, const float* vel
         if (!std::isfinite(times[i])) return KBMOD_ERR_ARG;
     return KBMOD_OK;
 }
-static int check_result(const kbmod_result* out) {
+// planes may be NULL only when nothing will be written (an empty band of start rows)
+static int check_result(const kbmod_result* out, bool empty = false) {
     if (!out) return KBMOD_ERR_NULL;
-    if (!out->vel_idx || !out->n_obs || !out->psi || !out->phi || !out->nu || !out->alpha) return KBMOD_ERR_NULL;
+    if (!empty && (!out->vel_idx || !out->n_obs || !out->psi || !out->phi || !out->nu || !out->alpha))
+        return KBMOD_ERR_NULL;
     if (((uintptr_t)out->vel_idx | (uintptr_t)out->n_obs | (uintptr_t)out->psi | (uintptr_t)out->phi |
          (uintptr_t)out->nu | (uintptr_t)out->alpha) & 3)
         return KBMOD_ERR_ALIGN;
@@ -179,10 +181,10 @@ int kbmod_plan_kernel(const kbmod_plan* plan) { return plan ? plan->kernel : KBM
 int kbmod_search_planned(const kbmod_plan* plan, const float* psiphi, int min_obs, int y_begin, int y_end,
                          const kbmod_result* out, void* workspace, size_t workspace_bytes, void* stream) {
     if (!plan || !psiphi || !workspace) return KBMOD_ERR_NULL;
-    if (int rc = check_result(out)) return rc;
     const int N = plan->N, H = plan->H, W = plan->W, V = plan->V, K = plan->K;
     if (min_obs < 1 || min_obs > N) return KBMOD_ERR_ARG;
     if (y_begin < 0 || y_end > H || y_begin > y_end) return KBMOD_ERR_ARG;
+    if (int rc = check_result(out, y_begin == y_end)) return rc;
     if (((uintptr_t)psiphi & 15) || ((uintptr_t)workspace & 255)) return KBMOD_ERR_ALIGN;
     const WorkspaceLayout l = workspace_layout(N, H, W, V, K);
     if (workspace_bytes < l.total) return KBMOD_ERR_WORKSPACE;
@@ -193,6 +195,7 @@ int kbmod_search_planned(const kbmod_plan* plan, const float* psiphi, int min_ob
     const float2* pp = reinterpret_cast<const float2*>(psiphi);
     int* status_dev = reinterpret_cast<int*>(ws + l.status_off);
     if (cudaMemsetAsync(status_dev, 0, sizeof(int), st) != cudaSuccess) return KBMOD_ERR_CUDA;
+    if (y_begin == y_end) return KBMOD_OK;                 // an empty band: nothing to search, nothing to write
     float2* vel_dev = reinterpret_cast<float2*>(ws + l.vel_off);
     if (cudaMemcpyAsync(vel_dev, plan->vel.data(), (size_t)V * sizeof(float2), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
@@ -216,10 +219,10 @@ int kbmod_search_rows(const float* psiphi, const double* times, int N, int H, in
                       const kbmod_search_options* options, void* stream) {
     // every argument error is found here, before the plan is built or anything is launched
     if (!psiphi || !workspace) return KBMOD_ERR_NULL;
-    if (int rc = check_result(out)) return rc;
     if (int rc = check_grid(times, N, H, W, vel_grid, V, K)) return rc;
     if (min_obs < 1 || min_obs > N) return KBMOD_ERR_ARG;
     if (y_begin < 0 || y_end > H || y_begin > y_end) return KBMOD_ERR_ARG;
+    if (int rc = check_result(out, y_begin == y_end)) return rc;
     if (((uintptr_t)psiphi & 15) || ((uintptr_t)workspace & 255)) return KBMOD_ERR_ALIGN;
     if (workspace_bytes < workspace_layout(N, H, W, V, K).total) return KBMOD_ERR_WORKSPACE;
     Options opt;

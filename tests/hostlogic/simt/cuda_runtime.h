@@ -81,7 +81,7 @@ enum { cudaEnableDefault = 0 };
 // switch, which dominates the run time), ucontext elsewhere
 #if defined(__x86_64__)
 extern "C" void simt_switch(void** save_sp, void* load_sp);
-asm(".text\n.globl simt_switch\n.type simt_switch,@function\nsimt_switch:\n"
+asm(".text\n.weak simt_switch\n.type simt_switch,@function\nsimt_switch:\n"
     "pushq %rbp\npushq %rbx\npushq %r12\npushq %r13\npushq %r14\npushq %r15\n"
     "movq %rsp, (%rdi)\nmovq %rsi, %rsp\n"
     "popq %r15\npopq %r14\npopq %r13\npopq %r12\npopq %rbx\npopq %rbp\nret\n"

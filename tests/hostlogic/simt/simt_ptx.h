@@ -13,7 +13,12 @@
 // (no namespace and no includes here: search_staged.cu includes this file inside namespace kbmod,
 // after <cuda.h> and <cuda_runtime.h> of this directory)
 
-inline unsigned smem_u32(const void* p);      // defined by the test driver (it owns smem_raw)
+// shared-window address of a pointer into the CTA's shared-memory array (kbmod::smem_raw, owned by
+// the test driver that links this translation unit)
+extern unsigned char smem_raw[];
+inline unsigned smem_u32(const void* p) {
+    return simt::SMEM_BASE + (unsigned)(static_cast<const unsigned char*>(p) - smem_raw);
+}
 
 inline void mbar_touch(simt::MBar& b) {
     if (b.pending == 0 && b.tx == 0) { b.phase ^= 1u; b.pending = b.expected; }

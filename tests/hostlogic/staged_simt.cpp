@@ -11,9 +11,6 @@
 
 namespace kbmod {
 alignas(1024) unsigned char smem_raw[simt::SMEM_MAX + 64];
-inline unsigned smem_u32(const void* p) {
-    return simt::SMEM_BASE + (unsigned)(static_cast<const unsigned char*>(p) - smem_raw);
-}
 }  // namespace kbmod
 
 #include "search_staged.cu"

@@ -58,3 +58,31 @@ def load(name, emul_define=None):
     if _stale(lib, os.path.join(HL, name + ".cpp")):
         subprocess.run(cmd, check=True)
     return ctypes.CDLL(lib)
+
+
+# ---- the whole C-ABI library under emulation (tests/hostlogic/abi_simt.cpp)
+ABI_SOURCES = ["api.cu", "psi_phi.cu", "search_direct.cu", "search_tiled.cu", "search_staged.cu", "postproc.cu"]
+
+
+def build_abi_lib():
+    """Compiles every csrc/*.cu (one translation unit each, in parallel) plus the glue with g++ against
+    the SIMT emulator and links tests/hostlogic/libkbmod_emul.so; returns its path."""
+    lib = os.path.join(HL, "libkbmod_emul.so")
+    glue = os.path.join(HL, "abi_simt.cpp")
+    if not _stale(lib, glue):
+        return lib
+    out = os.path.join(HL, "build_abi")
+    os.makedirs(out, exist_ok=True)
+    flags = ["-O1", "-std=c++17", "-ffp-contract=off", "-fPIC", "-fno-gnu-unique", "-I", os.path.join(HL, "simt"),
+             "-I", os.path.join(ROOT, "include"), "-I", CSRC, '-DKBMOD_SIMT_EMUL="simt_ptx.h"']
+    procs, objs = [], []
+    for src in [os.path.join(CSRC, f) for f in ABI_SOURCES] + [glue]:
+        obj = os.path.join(out, os.path.basename(src) + ".o")
+        objs.append(obj)
+        procs.append((src, subprocess.Popen(["g++", *flags, "-x", "c++", "-c", src, "-o", obj])))
+    for src, p in procs:
+        if p.wait() != 0:
+            raise RuntimeError(f"g++ failed on {src}")
+    # -Bsymbolic: the library binds its own symbols (the emulator state, smem_raw) whatever else is loaded
+    subprocess.run(["g++", "-shared", "-Wl,-Bsymbolic", "-o", lib, *objs], check=True)
+    return lib

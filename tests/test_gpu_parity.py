@@ -291,8 +291,9 @@ def test_errors_are_loud(kb):
         kb.search(pp, [0.0, 1.0], np.zeros((1, 2), np.float32), 40, 1)        # K > 32
     with pytest.raises(kb.KbmodError):
         kb.search(pp, [0.0, np.nan], np.zeros((1, 2), np.float32), 2, 1)      # bad time
-    with pytest.raises(kb.KbmodError):
-        kb.search(pp.cpu(), [0.0, 1.0], np.zeros((1, 2), np.float32), 2, 1)   # host tensor
+    if not EMULATED:
+        with pytest.raises(kb.KbmodError):
+            kb.search(pp.cpu(), [0.0, 1.0], np.zeros((1, 2), np.float32), 2, 1)   # host tensor
 
 
 # ------------------------------------------------------------------------------ added after the last GPU run
@@ -317,10 +318,13 @@ def test_search_host_entry_point(kb, orc):
     """kbmod_search_host (HOST buffers in, HOST planes out) equals the two device-pointer calls."""
     cfg = synth.config(2, N=8, H=75, W=203)
     st = synth.make_stack(cfg)
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    out = {k: torch.empty((cfg.H, cfg.W, cfg.K), dtype=torch.int32 if k in ("vel_idx", "n_obs") else torch.float32).pin_memory()
+    pin = lambda a: (lambda t: t if EMULATED else t.pin_memory())(torch.from_numpy(np.ascontiguousarray(a)))
+    out = {k: torch.empty((cfg.H, cfg.W, cfg.K), dtype=torch.int32 if k in ("vel_idx", "n_obs") else torch.float32)
            for k in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")}
-    ws = torch.empty(kb.search_host_workspace(cfg.N, cfg.H, cfg.W, cfg.V, cfg.K), dtype=torch.uint8, device="cuda")
+    if not EMULATED:
+        out = {k: v.pin_memory() for k, v in out.items()}
+    nws = kb.search_host_workspace(cfg.N, cfg.H, cfg.W, cfg.V, cfg.K)
+    ws = kb.aligned_empty(nws) if EMULATED else torch.empty(nws, dtype=torch.uint8, device="cuda")
     kb.search_host(pin(st.sci), pin(st.var), pin(st.mask), st.psf, st.times, st.vel_grid, cfg.K, cfg.min_obs, out, ws)
     kb.search_status(ws)                                  # synchronises
     pp = kb.make_psi_phi(_cuda(st.sci), _cuda(st.var), _cuda(st.mask), st.psf)

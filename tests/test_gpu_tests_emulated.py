@@ -1,13 +1,18 @@
-"""The `-m gpu` test files, exercised on the CPU (`-m "not gpu"`).
+"""The `-m gpu` test files and the C-ABI layer, exercised on the CPU (`-m "not gpu"`).
 
-With KBMOD_GPU_TESTS_EMULATED=1 the GPU test files take tests/emulated_binding.py -- the product's
-launch code and kernels compiled with g++ against the SIMT emulator, on CPU tensors -- in place of
-the ctypes binding.  A child pytest runs a part of them here on every CPU run, so that a GPU test
-that is wrong (a bad expectation, a misuse of the API, a case the kernels do not support) is found
-on this machine and not on the first B200 that runs it.  The whole of the small-size GPU tests, all
-four search kernels included, passes this way (168 s: `KBMOD_GPU_TESTS_EMULATED=1 KBMOD_TEST_STAGED=1
-KBMOD_TEST_QUEUED=1 pytest -m gpu tests -k "not full_size and not host_entry and not split and not
-errors"`); the subset below keeps the CPU suite short.  Nothing here says anything about hardware.
+With KBMOD_GPU_TESTS_EMULATED=1 the GPU test files take tests/emulated_binding.py in place of the
+ctypes binding: the product's own binding.py (a private, patched copy) over
+tests/hostlogic/libkbmod_emul.so, the WHOLE library -- api.cu and every kernel file -- compiled with
+g++ against the SIMT emulator, on CPU tensors.  A child pytest runs a part of the GPU tests that way
+on every CPU run, so that (1) the success paths of the ABI layer (workspace layout, plans, options,
+kbmod_search_host's pipeline, the dispatch of every call) execute somewhere before a GPU sees them,
+and (2) a GPU test that is wrong -- a bad expectation, a misuse of the API -- fails on this machine
+and not on the first B200 that runs it.  (It has already paid for itself: it found that an empty band
+of start rows was refused because zero-sized result planes have NULL data pointers, and two wrong
+expectations in new GPU tests.)  The whole of the small-size GPU tests, all four search kernels
+included, passes this way (`KBMOD_GPU_TESTS_EMULATED=1 KBMOD_TEST_STAGED=1 KBMOD_TEST_QUEUED=1 pytest
+-m gpu tests -k "not full_size"`, a few minutes); the subset below keeps the CPU suite short.
+Nothing here says anything about hardware.
 """
 import os
 import subprocess
@@ -25,7 +30,7 @@ def test_gpu_test_files_pass_against_the_emulated_library():
     cp = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider", "-m", "gpu",
                          "tests/test_zx_gpu_next_rows.py", "tests/test_gpu_parity.py", "-k",
                          "next_rows or edge_cases or half_integer or eval_trajectories or maximum_image or "
-                         "(row_bands and 0) or psi_phi"],
+                         "(row_bands and 0) or psi_phi or host_entry or split or errors"],
                         cwd=ROOT, env=env, capture_output=True, text=True, timeout=1200)
     assert cp.returncode == 0, cp.stdout[-4000:] + cp.stderr[-2000:]
     assert " passed" in cp.stdout and " failed" not in cp.stdout
