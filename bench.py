@@ -228,7 +228,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     bands = bool(args.bands) and world > 1
     y0, y1 = shard.row_bands(H, world)[rank] if bands else (0, H)
     out = binding.alloc_result(y1 - y0, W, K, dev)
-    ws = torch.empty(binding.search_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
+    ws = binding.alloc_workspace(binding.search_workspace(N, H, W, V, K), dev)
     h_out = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
     e_sci, e_var, e_mask = torch.empty_like(d_sci), torch.empty_like(d_var), torch.empty_like(d_mask)
     h_count = torch.zeros(1, dtype=torch.int64).pin_memory()
@@ -310,7 +310,7 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
     try:
         if world > 1 or args.mode == "threshold":
             raise RuntimeError("measured at N=1 in top-K mode only")
-        ws_h = torch.empty(binding.search_host_workspace(N, H, W, V, K), dtype=torch.uint8, device=dev)
+        ws_h = binding.alloc_workspace(binding.search_host_workspace(N, H, W, V, K), dev)
         run_h = lambda: binding.search_host(h_sci, h_var, h_mask, st.psf, st.times, st.vel_grid, K,
                                             cfg.min_obs, h_out, ws_h, kernel=kernel)
         run_h()

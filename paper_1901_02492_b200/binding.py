@@ -182,6 +182,12 @@ def search_workspace(N: int, H: int, W: int, V: int, K: int) -> int:
     return int(lib().kbmod_search_workspace(N, H, W, V, K))
 
 
+def alloc_workspace(nbytes: int, device) -> torch.Tensor:
+    """Device scratch for the calls that take a workspace (256-byte alignment is required; the CUDA
+    caching allocator aligns every block to 512 bytes)."""
+    return torch.empty(int(nbytes), dtype=torch.uint8, device=device)
+
+
 def make_psi_phi(sci: torch.Tensor, var: torch.Tensor, mask: Optional[torch.Tensor], psf,
                  out: Optional[torch.Tensor] = None) -> torch.Tensor:
     """kbmod_make_psi_phi: sci/var [N,H,W] f32 cuda, mask [N,H,W] u8 cuda or None, psf host
@@ -246,7 +252,7 @@ def search(psiphi: torch.Tensor, times, vel_grid, K: int, min_obs: int,
     need = search_workspace(N, H, W, V, K)
     own_workspace = workspace is None
     if own_workspace:
-        workspace = torch.empty(need, dtype=torch.uint8, device=psiphi.device)
+        workspace = alloc_workspace(need, psiphi.device)
     res = _result_struct(out, rows, W, int(K))
     if plan is not None:
         rc = lib().kbmod_search_planned(plan._h, _dev(psiphi, torch.float32, "psiphi"), int(min_obs), y_begin,
@@ -322,7 +328,7 @@ def search_split(psi: torch.Tensor, phi: torch.Tensor, times, vel_grid, K: int, 
     V = vel.shape[0]
     out = alloc_result(H, W, K, psi.device)
     need = search_workspace(N, H, W, V, K) + N * H * W * 8
-    ws = torch.empty(need, dtype=torch.uint8, device=psi.device)
+    ws = alloc_workspace(need, psi.device)
     res = _Result(*[ctypes.c_void_p(out[k].data_ptr()) for k in
                     ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")])
     rc = lib().kbmod_search_split(_dev(psi, torch.float32, "psi"), _dev(phi, torch.float32, "phi"),
@@ -380,7 +386,7 @@ def search_threshold(psiphi: torch.Tensor, times, vel_grid, min_obs: int, nu_min
     out.update({k: torch.empty(max(1, int(capacity)), dtype=torch.float32, device=dev) for k in _CAND_FLT})
     count = torch.zeros(1, dtype=torch.int64, device=dev)
     if workspace is None:
-        workspace = torch.empty(search_workspace(N, H, W, V, 8), dtype=torch.uint8, device=dev)
+        workspace = alloc_workspace(search_workspace(N, H, W, V, 8), dev)
     cand = _Candidates(*[ctypes.c_void_p(out[k].data_ptr()) for k in _CAND_INT + _CAND_FLT])
     opt = _options(kernel, tile_group_w)
     rc = lib().kbmod_search_threshold(_dev(psiphi, torch.float32, "psiphi"), times.ctypes.data_as(ctypes.c_void_p),
@@ -460,7 +466,7 @@ def cluster_candidates(x0y0: torch.Tensor, vxvy: torch.Tensor, nu: torch.Tensor,
     dev = x0y0.device
     label = torch.empty(M, dtype=torch.int32, device=dev)
     rep = torch.empty(M, dtype=torch.uint8, device=dev)
-    ws = torch.empty(int(lib().kbmod_cluster_workspace(M)), dtype=torch.uint8, device=dev)
+    ws = alloc_workspace(lib().kbmod_cluster_workspace(M), dev)
     rc = lib().kbmod_cluster_candidates(_dev(x0y0, torch.int32, "x0y0"), _dev(vxvy, torch.float32, "vxvy"),
                                         _dev(nu, torch.float32, "nu"), M, ctypes.c_float(eps_xy), ctypes.c_float(eps_v),
                                         int(min_samples), ctypes.c_void_p(label.data_ptr()), ctypes.c_void_p(rep.data_ptr()),

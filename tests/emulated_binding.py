@@ -51,20 +51,7 @@ def aligned_empty(n, align=256):
     return raw[off:off + int(n)]
 
 
-class _Torch:
-    """`torch` as the patched binding sees it: workspaces (1-D uint8) come out 256-byte aligned."""
-
-    def __getattr__(self, name):
-        return getattr(_torch, name)
-
-    @staticmethod
-    def empty(*size, dtype=None, device=None, **kw):
-        if dtype == _torch.uint8 and len(size) == 1 and isinstance(size[0], int):
-            return aligned_empty(size[0])
-        return _torch.empty(*size, dtype=dtype, device=device, **kw)
-
-
-_b.torch = _Torch()
+_b.alloc_workspace = lambda nbytes, device=None: aligned_empty(nbytes)
 
 # the public names of the binding, served by the patched copy
 for _name in dir(_b):

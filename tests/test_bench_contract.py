@@ -47,6 +47,7 @@ def stubbed(monkeypatch):
                                            for k in planes}
     b.search_workspace = lambda *a: 1024
     b.search_host_workspace = lambda *a: 2048
+    b.alloc_workspace = lambda n, dev=None: torch.empty(int(n), dtype=torch.uint8)
 
     def make_psi_phi(*a, out=None, **k):
         calls["launches"] += 1
@@ -144,6 +145,26 @@ def test_threshold_mode_line(stubbed, monkeypatch):
     d = run_main(monkeypatch, ["--config", "1", "--steps", "2", "--mode", "threshold", "--nu-min", "7", "--no-cpu"])
     assert stubbed["threshold"] >= 2 + 3 and "kbmod_search_threshold" in d["config"]["step"]
     assert d["e2e"]["d2h_bytes_per_step"] == 8 and d["gpu_launches"] == 4
+
+
+def test_gpu_arm_against_the_emulated_library(stubbed, monkeypatch):
+    """bench.py's GPU arm with the REAL calls: the stub binding is replaced by tests/emulated_binding.py
+    (the product's binding over the SIMT-emulated library), so bench.py's use of kbmod_plan,
+    kbmod_search_planned, kbmod_search_host and kbmod_search_threshold runs for real on config 1.
+    Only the torch.cuda calls stay stubbed.  Timings mean nothing."""
+    from tests import emulated_binding
+    import paper_1901_02492_b200
+    monkeypatch.setitem(sys.modules, "paper_1901_02492_b200.binding", emulated_binding)
+    monkeypatch.setattr(paper_1901_02492_b200, "binding", emulated_binding, raising=False)
+    d = run_main(monkeypatch, ["--config", "1", "--steps", "1", "--warmup", "1", "--no-cpu"])
+    assert d["gpu_launches"] == 3                      # psi/phi (one launch for the stack) + encode + search
+    assert d["e2e_host_abi"].get("verified_equal_to_resident_run") is True
+    assert "kbmod_search_host" in d["e2e"]["path"]
+    for k in (1, 3, 4):
+        d = run_main(monkeypatch, ["--config", "1", "--steps", "1", "--kernel", str(k), "--no-cpu"])
+        assert d["search_options"]["kernel"] == k and d["e2e_host_abi"].get("verified_equal_to_resident_run") is True
+    d = run_main(monkeypatch, ["--config", "1", "--steps", "1", "--mode", "threshold", "--nu-min", "5", "--no-cpu"])
+    assert "kbmod_search_threshold" in d["config"]["step"] and d["gpu_launches"] == 2
 
 
 def test_reference_arm_line(monkeypatch):

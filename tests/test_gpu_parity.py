@@ -323,8 +323,7 @@ def test_search_host_entry_point(kb, orc):
            for k in ("vel_idx", "n_obs", "psi", "phi", "nu", "alpha")}
     if not EMULATED:
         out = {k: v.pin_memory() for k, v in out.items()}
-    nws = kb.search_host_workspace(cfg.N, cfg.H, cfg.W, cfg.V, cfg.K)
-    ws = kb.aligned_empty(nws) if EMULATED else torch.empty(nws, dtype=torch.uint8, device="cuda")
+    ws = kb.alloc_workspace(kb.search_host_workspace(cfg.N, cfg.H, cfg.W, cfg.V, cfg.K), "cpu" if EMULATED else "cuda")
     kb.search_host(pin(st.sci), pin(st.var), pin(st.mask), st.psf, st.times, st.vel_grid, cfg.K, cfg.min_obs, out, ws)
     kb.search_status(ws)                                  # synchronises
     pp = kb.make_psi_phi(_cuda(st.sci), _cuda(st.var), _cuda(st.mask), st.psf)
