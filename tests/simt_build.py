@@ -40,23 +40,43 @@ def build_command(name, sanitize=SANITIZE):
     return lib, cmd
 
 
+_running = {}        # library path -> Popen of the g++ that is building it (this process started it)
+
+
+def _start(name, sanitize):
+    lib, cmd = build_command(name, sanitize)
+    if lib not in _running and _stale(lib, os.path.join(HL, name + ".cpp")):
+        _running[lib] = subprocess.Popen(cmd)
+    return lib
+
+
+def _wait(lib, what):
+    p = _running.pop(lib, None)
+    if p is not None and p.wait() != 0:
+        raise RuntimeError(f"g++ failed on {what}")
+
+
+def start_background_builds(sanitized=True):
+    """Starts every stale harness build at once and returns immediately (tests/conftest.py calls this
+    at session start, so the compilers run while the first tests do); load() / build_all() wait for
+    the library they need."""
+    for name in HARNESSES:
+        _start(name, False)
+        if sanitized:
+            _start(name, True)
+
+
 def build_all(sanitize=SANITIZE):
     """Compiles every stale harness of one flavour, all at once (they are independent translation units)."""
-    procs = []
-    for name in HARNESSES:
-        lib, cmd = build_command(name, sanitize)
-        if _stale(lib, os.path.join(HL, name + ".cpp")):
-            procs.append((name, subprocess.Popen(cmd)))
-    for name, p in procs:
-        if p.wait() != 0:
-            raise RuntimeError(f"g++ failed on {name}")
+    libs = [(name, _start(name, sanitize)) for name in HARNESSES]
+    for name, lib in libs:
+        _wait(lib, name)
 
 
 def load(name, emul_define=None):
     """Compiles tests/hostlogic/<name>.cpp if stale and loads it."""
-    lib, cmd = build_command(name)
-    if _stale(lib, os.path.join(HL, name + ".cpp")):
-        subprocess.run(cmd, check=True)
+    lib = _start(name, SANITIZE)
+    _wait(lib, name)
     return ctypes.CDLL(lib)
 
 
