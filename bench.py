@@ -196,7 +196,8 @@ def config_dict(cfg, args):
             "step": ("kbmod_make_psi_phi + kbmod_search_threshold (S1..S5 + nu >= %g, row N4)" % args.nu_min
                      if getattr(args, "mode", "topk") == "threshold" else "kbmod_make_psi_phi + kbmod_search (S1..S6)"),
             "l2": "inputs larger than L2 (stack 2.0 GB+ vs 126 MB); no flush needed",
-            "parallelism": (f"one stack, start-row bands x{args.gpus} (kbmod_search_rows)" if getattr(args, "bands", False)
+            "parallelism": (f"one stack: psi/phi sharded by image + one NCCL all-gather, then start-row bands x{args.gpus} "
+                            "(kbmod_search_rows)" if getattr(args, "bands", False)
                             and args.gpus > 1 else f"independent stacks x{args.gpus}")}
 
 
@@ -239,15 +240,21 @@ def run_gpu(args, cfg, st, rank, world, local_rank):
                                             y_begin=y0, y_end=y1, kernel=kernel, tile_group_w=args.group_w, workspace=ws)
         return binding.search(psiphi, None, None, K, cfg.min_obs, out=out, workspace=ws, plan=plan, y_begin=y0, y_end=y1)
 
+    def build_psi_phi(a, b, c):
+        if bands:       # one stack on all ranks: S2 sharded by image, one all-gather (NCCL), then the row-band search
+            psiphi.copy_(shard.make_psi_phi_sharded(a, b, c, st.psf))
+        else:
+            binding.make_psi_phi(a, b, c, st.psf, out=psiphi)
+
     def step_resident():
-        binding.make_psi_phi(d_sci, d_var, d_mask, st.psf, out=psiphi)
+        build_psi_phi(d_sci, d_var, d_mask)
         search_step()
 
     def step_e2e():
         e_sci.copy_(h_sci, non_blocking=True)
         e_var.copy_(h_var, non_blocking=True)
         e_mask.copy_(h_mask, non_blocking=True)
-        binding.make_psi_phi(e_sci, e_var, e_mask, st.psf, out=psiphi)
+        build_psi_phi(e_sci, e_var, e_mask)
         r = search_step()
         if args.mode == "threshold":
             h_count.copy_(r[0], non_blocking=True)          # the candidate list stays on the device for N1/N2

@@ -90,3 +90,34 @@ def search_row_band(psiphi, times, vel_grid, K: int, min_obs: int, search: Optio
     y0, y1 = row_bands(H, n)[rank]
     band = search(psiphi, times, vel_grid, K, min_obs, y_begin=y0, y_end=y1, **kw)
     return gather_bands(band, H) if gather else band
+
+
+def image_shares(N: int, world_size: int) -> List[Tuple[int, int]]:
+    """Balanced contiguous shares [i0, i1) of the N images, one per rank (S2 sharded by image)."""
+    return row_bands(N, world_size)
+
+
+def make_psi_phi_sharded(sci: torch.Tensor, var: torch.Tensor, mask: Optional[torch.Tensor], psf,
+                         make: Optional[Callable] = None) -> torch.Tensor:
+    """S1+S2 of ONE stack on all ranks: rank r builds psi/phi of its share of
+    the images (kbmod_make_psi_phi on a slice of the stack) and ONE all-gather (NCCL over NVLink on
+    GPUs, gloo in the CPU tests) replicates the float2 stack on every rank, ready for the row-band
+    search.  This is the only exchange step of the multi-GPU path; images are independent, so the
+    gathered stack is bit-identical to a single-rank build.  `make` defaults to binding.make_psi_phi."""
+    if make is None:
+        from . import binding
+        make = binding.make_psi_phi
+    rank, n = world()
+    N, H, W = sci.shape
+    if n == 1:
+        return make(sci, var, mask, psf)
+    shares = image_shares(N, n)
+    i0, i1 = shares[rank]
+    cmax = max(b - a for a, b in shares)
+    part = torch.zeros((cmax, H, W, 2), dtype=torch.float32, device=sci.device)
+    if i1 > i0:
+        part[: i1 - i0] = make(sci[i0:i1].contiguous(), var[i0:i1].contiguous(),
+                               None if mask is None else mask[i0:i1].contiguous(), psf[i0:i1])
+    parts = [torch.empty_like(part) for _ in range(n)]
+    dist.all_gather(parts, part)
+    return torch.cat([p[: b - a] for p, (a, b) in zip(parts, shares)], 0).contiguous()

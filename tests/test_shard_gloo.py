@@ -45,6 +45,17 @@ def _worker(rank, world, port, ret):
         for k in ref:
             a, b = full[k].numpy(), ref[k]
             assert a.shape == b.shape and ((a == b) | (np.isnan(a) & np.isnan(b))).all(), k
+        # S2 sharded by image + one all-gather: bit-identical to a single-rank build (emulated kernel)
+        from tests import emulated_binding
+        cfg = synth.config(2, N=5, H=40, W=68, n_sources=2)
+        st = synth.make_stack(cfg)
+        tens = lambda a: torch.from_numpy(np.ascontiguousarray(a))
+        whole = emulated_binding.make_psi_phi(tens(st.sci), tens(st.var), tens(st.mask), st.psf)
+        gathered = shard.make_psi_phi_sharded(tens(st.sci), tens(st.var), tens(st.mask), st.psf,
+                                              make=emulated_binding.make_psi_phi)
+        assert gathered.shape == whole.shape
+        assert torch.equal(gathered.view(torch.int32), whole.view(torch.int32))
+        assert shard.image_shares(5, world) == [(0, 3), (3, 5)]
         t = shard.max_over_ranks(10.0 + 5.0 * rank)
         n = shard.total_over_ranks(100.0 * (rank + 1))
         assert t == 10.0 + 5.0 * (world - 1) and n == 100.0 * world * (world + 1) / 2
@@ -74,6 +85,7 @@ def test_world_size_2_gloo(orc):
     port = _free_port()
     from tests import simt_build
     simt_build.load("tiled_simt")            # compile once, before the ranks race for it
+    simt_build.build_abi_lib()
     procs = [ctx.Process(target=_worker, args=(r, 2, port, ret)) for r in range(2)]
     for p in procs:
         p.start()
