@@ -43,6 +43,35 @@ inline std::vector<std::pair<unsigned, int>> hilbert_order(const float* vel, int
     return key;
 }
 
+// Row pitch (in samples) of the encoded stack: W rounded up to even, so that every row starts
+// 16-byte aligned and a pair of samples never straddles two rows.
+__host__ __device__ constexpr int enc_pitch(int W) { return (W + 1) & ~1; }
+
+// The encoded stack of the tiled and staged kernels: (psi, phi) -> (psi, -phi), invalid (psi NaN) ->
+// (+0, +0); rows padded to Wp = enc_pitch(W) samples, the padding column is zero.  Adding a zero is
+// exact, so one packed add per sample yields the in-order fp32 sums of both planes over the valid
+// observations, and the sign bit of the second word is the validity flag.  One thread per pair.
+__global__ void __launch_bounds__(256)
+inline encode_kernel(const float2* __restrict__ in, float4* __restrict__ out, int W, int Wp, size_t rows) {
+    const int half = Wp >> 1;
+    const size_t total = rows * (size_t)half;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
+        const size_t row = k / half;
+        const int x = (int)(k - row * half) * 2;
+        const float2* src = in + row * W + x;
+        const float2 a = __ldg(src);
+        const float2 b = (x + 1 < W) ? __ldg(src + 1) : make_float2(__int_as_float(0x7FC00000), 0.0f);
+        const bool va = (a.x == a.x), vb = (b.x == b.x);
+        float4 o;
+        o.x = va ? a.x : 0.0f;
+        o.y = va ? -a.y : 0.0f;
+        o.z = vb ? b.x : 0.0f;
+        o.w = vb ? -b.y : 0.0f;
+        out[k] = o;
+    }
+}
+
 }  // namespace kbmod
 
 // One step S of the S5 pre-test / queue switch of the queued kernels (kernels 3 and 4): trajectory

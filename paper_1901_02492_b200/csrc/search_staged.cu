@@ -269,7 +269,7 @@ size_t staged_plan_bytes(int N, int V) {
     const size_t nblk = ((size_t)V + B - 1) / B;
     return nblk * ((size_t)std::max(N - 1, 0) * B + 1) * HDR_INTS * sizeof(int) + 256;
 }
-size_t staged_enc_bytes(int N, int H, int W) { return (size_t)N * H * ((W + 1) & ~1) * sizeof(float2); }
+size_t staged_enc_bytes(int N, int H, int W) { return (size_t)N * H * enc_pitch(W) * sizeof(float2); }
 
 int staged_plan_build(const DtTable& dt, int N, int H, int W, const float* vel_host, int V, int geom,
                       StagedPlan& plan) {
@@ -302,29 +302,6 @@ int staged_plan_debug(const DtTable& dt, int N, int H, int W, const float* vel_h
 // device side
 // ---------------------------------------------------------------------------------------------
 typedef unsigned long long u64;
-
-// (psi, phi) -> (psi, -phi), invalid (psi NaN) -> (+0, +0); rows padded to Wp (even) samples, the
-// padding column is zero.  One thread per pair of samples.
-__global__ void __launch_bounds__(256)
-encode_kernel(const float2* __restrict__ in, float4* __restrict__ out, int W, int Wp, size_t rows) {
-    const int half = Wp >> 1;
-    const size_t total = rows * (size_t)half;
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
-        const size_t row = k / half;
-        const int x = (int)(k - row * half) * 2;
-        const float2* src = in + row * W + x;
-        const float2 a = __ldg(src);
-        const float2 b = (x + 1 < W) ? __ldg(src + 1) : make_float2(__int_as_float(0x7FC00000), 0.0f);
-        const bool va = (a.x == a.x), vb = (b.x == b.x);
-        float4 o;
-        o.x = va ? a.x : 0.0f;
-        o.y = va ? -a.y : 0.0f;
-        o.z = vb ? b.x : 0.0f;
-        o.w = vb ? -b.y : 0.0f;
-        out[k] = o;
-    }
-}
 
 // The inline-PTX helpers.  tests/test_staged_simt.py compiles this file with g++ against a SIMT
 // emulator (tests/hostlogic/simt/) and defines KBMOD_SIMT_EMUL as the header that supplies host
@@ -832,7 +809,7 @@ int staged_launch(const StagedPlan& plan, const float2* psiphi, const DtTable& d
         return KBMOD_ERR_CUDA;
 
     if (cudaMemsetAsync(status_dev, 0, sizeof(int), st) != cudaSuccess) return KBMOD_ERR_CUDA;
-    const int Wp = (W + 1) & ~1;
+    const int Wp = enc_pitch(W);
     KBMOD_LAUNCH(encode_kernel, 148 * 8, 256, 0, st, psiphi, reinterpret_cast<float4*>(enc_dev), W, Wp, (size_t)N * H);
     note_launch();
     if (cudaGetLastError() != cudaSuccess) return KBMOD_ERR_CUDA;

@@ -13,7 +13,7 @@
 //     warp read 32 consecutive float2 samples at  base + offset[j][i]: one IMAD.WIDE + LDG.64 per
 //     sample, no per-lane position arithmetic and no bounds test (the host-side bounding box of a
 //     velocity's shifts decides once per (tile, velocity) whether every window is inside).
-//   * The stack is re-encoded once per call as (psi, -phi) with invalid samples = (+0,+0): one
+//   * The stack is re-encoded once per call (search_common.cuh) as (psi, -phi) with invalid samples = (+0,+0): one
 //     packed add.rn.f32x2 accumulates both sums (adding +0 / -0 is exact, so the result equals the
 //     in-order fp32 sum over valid observations), and the sign bit of the second word is the
 //     validity flag, counted with one LEA.HI.  3 instructions per sample.
@@ -68,7 +68,7 @@ int tiled_plan_build(const DtTable& dt, int N, int H, int W, const float* vel_ho
     // limits of the int16 shift encoding and of the int32 element offsets
     if (W > 30000 || H > 30000) return KBMOD_ERR_UNSUPPORTED;
     if (queued && V >= (1 << 24)) return KBMOD_ERR_UNSUPPORTED;    // 25-bit velocity index in the queue word
-    if ((long long)(N + 1) * H * W + (long long)SH_LIMIT * (W + 1) >= 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
+    if ((long long)(N + 1) * H * enc_pitch(W) + (long long)SH_LIMIT * (enc_pitch(W) + 1) >= 0x7FFFFFFFLL) return KBMOD_ERR_UNSUPPORTED;
     plan.queued = queued;
     plan.nblk = build_plan(dt, N, H, W, vel_host, V, block_size_for_k(K), plan.rec, queued);
     if (plan.rec.size() * sizeof(int) > tiled_plan_bytes(N, V, K)) return KBMOD_ERR_UNSUPPORTED;
@@ -84,6 +84,7 @@ int tiled_plan_build(const DtTable& dt, int N, int H, int W, const float* vel_ho
 static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, int V, int B,
                       std::vector<int>& plan, bool isolate) {
     const std::vector<std::pair<unsigned, int>> key = hilbert_order(vel, V);    // processing order
+    const int Wp = enc_pitch(W);        // row pitch of the encoded stack the element offsets refer to
 
     // largest coordinate magnitude any fl(x0 + d) can reach for an in-range window
     const double cmax = 2.0 * std::max(W, H) + 4.0;
@@ -139,7 +140,7 @@ static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, 
             if (j == PAD_BENIGN) {               // never scored; samples the thread's own pixel of image i
                 m[0] = -1; m[1] = 0; m[2] = 0; m[3] = 1;
                 for (int i = 0; i < N; ++i) {
-                    off[b * N + i] = (int)((long long)i * H * W);
+                    off[b * N + i] = (int)((long long)i * H * Wp);
                     sh[b * N + i] = 0;           // proven shift (0, 0)
                 }
                 continue;
@@ -165,7 +166,7 @@ static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, 
                     } else {
                         const int sx = (int)std::floor(dx + 0.5), sy = (int)std::floor(dy + 0.5);
                         code = (int)(((unsigned)sy << 16) | ((unsigned)sx & 0xFFFFu));
-                        o = (long long)i * H * W + (long long)sy * W + sx;
+                        o = (long long)i * H * Wp + (long long)sy * Wp + sx;
                         if (i >= 1) {
                             sxlo = std::min(sxlo, sx); sxhi = std::max(sxhi, sx);
                             sylo = std::min(sylo, sy); syhi = std::max(syhi, sy);
@@ -189,28 +190,6 @@ static int build_plan(const DtTable& dt, int N, int H, int W, const float* vel, 
 // device side
 // ---------------------------------------------------------------------------------------------
 
-// (psi, phi) -> (psi, -phi), invalid (psi NaN) -> (+0, +0).  Two pixels per thread (float4).
-__global__ void __launch_bounds__(256)
-encode_kernel(const float4* __restrict__ in, float4* __restrict__ out, size_t n2,
-              const float2* __restrict__ in1, float2* __restrict__ out1, size_t n) {
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n2; k += stride) {
-        float4 v = __ldg(in + k);
-        float4 o;
-        const bool a = (v.x == v.x), b = (v.z == v.z);
-        o.x = a ? v.x : 0.0f;
-        o.y = a ? -v.y : 0.0f;
-        o.z = b ? v.z : 0.0f;
-        o.w = b ? -v.w : 0.0f;
-        out[k] = o;
-    }
-    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {   // odd tail pixel
-        const float2 v = in1[n - 1];
-        const bool a = (v.x == v.x);
-        out1[n - 1] = make_float2(a ? v.x : 0.0f, a ? -v.y : 0.0f);
-    }
-}
-
 typedef unsigned long long u64;
 
 __device__ __forceinline__ void acc_add(u64& a, u64 s) {      // (Psi, -Phi) += (psi, -phi), RN each
@@ -230,6 +209,7 @@ struct TiledParams {
     const int* plan;          // nblk records
     const float2* vel;        // caller's velocity table (device copy)
     int nblk, N, H, W, K, min_obs;
+    int Wp;                   // row pitch of the encoded stack (W rounded up to even)
     int y_begin, y_end;       // band of start rows; the result planes hold rows y_begin..y_end-1 only
     int tiles_x, tiles_y, group_w;
     kbmod_result out;
@@ -290,7 +270,7 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
     const u64* basep[RY];
 #pragma unroll
     for (int ry = 0; ry < RY; ++ry)
-        basep[ry] = prm.enc + (size_t)min(y_first + ry, H - 1) * W + min(x_first, W - 1);
+        basep[ry] = prm.enc + (size_t)min(y_first + ry, H - 1) * prm.Wp + min(x_first, W - 1);
 
     // per-pixel list state: nu of the worst entry (the K-th best once the list is full)
     float w_nu[R];
@@ -357,7 +337,7 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
                 } else {
                     const int code = r_sh[b * N + i];
                     if (code == SH_SKIP) continue;
-                    const u64* img = prm.enc + (size_t)i * H * W;
+                    const u64* img = prm.enc + (size_t)i * H * prm.Wp;
                     if (code != SH_UNSAFE) {
                         const int sx = (short)(code & 0xFFFF), sy = code >> 16;
                         // whole window outside: nothing to add (uniform over the CTA)
@@ -371,7 +351,7 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
                             for (int rx = 0; rx < RX; ++rx) {
                                 const int x = x_first + 32 * rx + sx;
                                 const bool in = yin && (x_first + 32 * rx < W) && x >= 0 && x < W;
-                                const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
+                                const u64 s = in ? ld_sample(img + (size_t)y * prm.Wp + x) : 0ull;
                                 acc_add(acc[b][ry * RX + rx], s);
                                 cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
                             }
@@ -389,7 +369,7 @@ search_tiled_kernel(const __grid_constant__ TiledParams prm) {
                                 int x = 0;
                                 const bool in = traj_pixel(x_first + 32 * rx, vx, dti, W, x) && yin &&
                                                 (x_first + 32 * rx < W);
-                                const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
+                                const u64 s = in ? ld_sample(img + (size_t)y * prm.Wp + x) : 0ull;
                                 acc_add(acc[b][ry * RX + rx], s);
                                 cnt[b][ry * RX + rx] += (unsigned)(s >> 63);
                             }
@@ -599,7 +579,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
     const u64* basep[RY];
 #pragma unroll
     for (int ry = 0; ry < RY; ++ry)
-        basep[ry] = prm.enc + (size_t)min(y_first + ry, H - 1) * W + min(x_first, W - 1);
+        basep[ry] = prm.enc + (size_t)min(y_first + ry, H - 1) * prm.Wp + min(x_first, W - 1);
 
 #if !defined(KBMOD_SIMT_EMUL)
     // keep the row pointers as opaque 64-bit registers: `basep[ry] + o` is then one IMAD.WIDE per
@@ -741,7 +721,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
                 } else {
                     const int code = r_sh[b * N + i];
                     if (code == SH_SKIP) continue;
-                    const u64* img = prm.enc + (size_t)i * H * W;
+                    const u64* img = prm.enc + (size_t)i * H * prm.Wp;
                     if (code != SH_UNSAFE) {
                         const int sx = (short)(code & 0xFFFF), sy = code >> 16;
                         // whole window outside: nothing to add (uniform over the CTA)
@@ -755,7 +735,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
                             for (int rx = 0; rx < RX; ++rx) {
                                 const int x = x_first + 32 * rx + sx;
                                 const bool in = yin && (x_first + 32 * rx < W) && x >= 0 && x < W;
-                                const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
+                                const u64 s = in ? ld_sample(img + (size_t)y * prm.Wp + x) : 0ull;
                                 take(b, ry * RX + rx, s);
                             }
                         }
@@ -772,7 +752,7 @@ search_tiledq_kernel(const __grid_constant__ TiledParams prm) {
                                 int x = 0;
                                 const bool in = traj_pixel(x_first + 32 * rx, vx, dti, W, x) && yin &&
                                                 (x_first + 32 * rx < W);
-                                const u64 s = in ? ld_sample(img + (size_t)y * W + x) : 0ull;
+                                const u64 s = in ? ld_sample(img + (size_t)y * prm.Wp + x) : 0ull;
                                 take(b, ry * RX + rx, s);
                             }
                         }
@@ -899,9 +879,8 @@ int tiled_launch(const TiledPlan& plan, const float2* psiphi, const DtTable& dt,
     if (cudaMemcpyAsync(plan_dev, plan.rec.data(), plan.rec.size() * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
 
-    const size_t n = (size_t)N * H * W;
-    KBMOD_LAUNCH(encode_kernel, 148 * 8, 256, 0, st, reinterpret_cast<const float4*>(psiphi),
-                 reinterpret_cast<float4*>(enc_dev), n / 2, psiphi, enc_dev, n);
+    KBMOD_LAUNCH(encode_kernel, 148 * 8, 256, 0, st, psiphi, reinterpret_cast<float4*>(enc_dev), W, enc_pitch(W),
+                 (size_t)N * H);
     note_launch();
     if (cudaGetLastError() != cudaSuccess) return KBMOD_ERR_CUDA;
 
@@ -911,6 +890,7 @@ int tiled_launch(const TiledPlan& plan, const float2* psiphi, const DtTable& dt,
     prm.plan = static_cast<const int*>(plan_dev);
     prm.vel = vel_dev;
     prm.nblk = plan.nblk; prm.N = N; prm.H = H; prm.W = W; prm.K = K; prm.min_obs = min_obs;
+    prm.Wp = enc_pitch(W);
     prm.y_begin = y_begin; prm.y_end = y_end;
     prm.out = out;
     prm.dt = dt;
@@ -934,9 +914,8 @@ int tiled_launch_threshold(const TiledPlan& plan, const float2* psiphi, const Dt
     if (!plan.queued) return KBMOD_ERR_ARG;
     if (cudaMemcpyAsync(plan_dev, plan.rec.data(), plan.rec.size() * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return KBMOD_ERR_CUDA;
-    const size_t n = (size_t)N * H * W;
-    KBMOD_LAUNCH(encode_kernel, 148 * 8, 256, 0, st, reinterpret_cast<const float4*>(psiphi),
-                 reinterpret_cast<float4*>(enc_dev), n / 2, psiphi, enc_dev, n);
+    KBMOD_LAUNCH(encode_kernel, 148 * 8, 256, 0, st, psiphi, reinterpret_cast<float4*>(enc_dev), W, enc_pitch(W),
+                 (size_t)N * H);
     note_launch();
     if (cudaGetLastError() != cudaSuccess) return KBMOD_ERR_CUDA;
     TiledParams prm;
@@ -946,6 +925,7 @@ int tiled_launch_threshold(const TiledPlan& plan, const float2* psiphi, const Dt
     prm.plan = static_cast<const int*>(plan_dev);
     prm.vel = vel_dev;
     prm.nblk = plan.nblk; prm.N = N; prm.H = H; prm.W = W; prm.K = 8; prm.min_obs = min_obs;   // plan blocks of 8
+    prm.Wp = enc_pitch(W);
     prm.y_begin = y_begin; prm.y_end = y_end;
     prm.dt = dt;
     prm.cand = cand; prm.capacity = capacity; prm.count = count; prm.nu_min = nu_min;

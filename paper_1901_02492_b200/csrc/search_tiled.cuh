@@ -24,7 +24,7 @@ int tiled_plan_build(const DtTable& dt, int N, int H, int W, const float* vel_ho
 
 // S3..S6 over the start rows [y_begin, y_end) with a prebuilt plan.  The result planes hold the band
 // only ([(y_end - y_begin)][W][K]).  plan_dev / enc_dev are carved from the caller's workspace
-// (tiled_plan_bytes() and N*H*W*8 bytes); vel_dev is the device copy of the velocity table.
+// (tiled_plan_bytes() and N*H*enc_pitch(W)*8 bytes, search_common.cuh); vel_dev is the device copy of the velocity table.
 // plan.queued = false: search_tiled_kernel (per-pixel lists in shared memory); true: search_tiledq_kernel
 // (same gathers; survivors of the pre-test compacted into per-warp queues, lists in the output planes).
 // group_w: tile columns per rasterisation group, 0 = default (kbmod_search_options.tile_group_w).

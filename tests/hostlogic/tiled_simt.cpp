@@ -40,7 +40,7 @@ int simt_search_tiled(const float* psiphi, const double* times, int N, int H, in
     // (devmem.h): inputs copied in, result planes copied back
     const size_t npix = (size_t)N * H * W, nres = (size_t)(y_end - y_begin) * W * K;
     simt::DevBuf d_pp(psiphi, npix * 8), d_vel(vel_grid, (size_t)V * 8);
-    simt::DevBuf d_plan(tiled_plan_bytes(N, V, K)), d_enc(npix * 8);
+    simt::DevBuf d_plan(tiled_plan_bytes(N, V, K)), d_enc((size_t)N * H * enc_pitch(W) * 8);
     simt::DevBuf d_vi(nres * 4), d_no(nres * 4), d_psi(nres * 4), d_phi(nres * 4), d_nu(nres * 4), d_al(nres * 4);
     kbmod_result out{d_vi.as<int32_t>(), d_no.as<int32_t>(), d_psi.as<float>(), d_phi.as<float>(),
                      d_nu.as<float>(), d_al.as<float>()};
@@ -69,7 +69,7 @@ long long simt_search_tiled_threshold(const float* psiphi, const double* times, 
     for (int i = 0; i < N; ++i) dt.dt[i] = (float)(times[i] - times[0]);
     const size_t npix = (size_t)N * H * W, nc = (size_t)capacity * 4;
     simt::DevBuf d_pp(psiphi, npix * 8), d_vel(vel_grid, (size_t)V * 8), d_count(8);
-    simt::DevBuf d_plan(tiled_plan_bytes(N, V, 8)), d_enc(npix * 8);
+    simt::DevBuf d_plan(tiled_plan_bytes(N, V, 8)), d_enc((size_t)N * H * enc_pitch(W) * 8);
     simt::DevBuf d_x(nc), d_y(nc), d_vi(nc), d_no(nc), d_psi(nc), d_phi(nc), d_nu(nc), d_al(nc);
     *d_count.as<unsigned long long>() = 0;
     kbmod_candidates out{d_x.as<int32_t>(), d_y.as<int32_t>(), d_vi.as<int32_t>(), d_no.as<int32_t>(), d_psi.as<float>(),
