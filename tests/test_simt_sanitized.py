@@ -56,6 +56,9 @@ def children(tmp_path_factory):
     if rt is None:
         pytest.skip("gcc has no libasan.so on this machine")
     simt_build.build_all(sanitize=True)                 # the three harnesses, compiled side by side
+    # the sanitized oracle is built ONCE here: every child loads it, none may find it half written
+    subprocess.run([sys.executable, "-c", "import oracle; oracle.build()"], cwd=ROOT, check=True,
+                   env=dict(os.environ, KBMOD_ORACLE_SANITIZE="1"))
     d = tmp_path_factory.mktemp("sanitized")
     procs = {}
     for name, args in CHILDREN.items():
