@@ -200,3 +200,39 @@ def test_plan_maximum_image_count(orc):
         times = np.sort(rng.uniform(0.0, 5.0, N))
         vel = synth.velocity_grid(6, 4, -math.pi / 2, math.pi / 2, 1.0, 9.0)
         check_against_oracle(orc, pp, times, vel)
+
+
+def test_fill_bytes_per_sample_byte_at_the_bench_workload():
+    """The numbers of DESIGN.md section 5.2, recomputed: bytes the staged kernel's plan moves into shared
+    memory per algorithmic sample byte at BASELINE.json configs[2] (15 x 4096 x 4096, 640 velocities),
+    against the floor no grouping into boxes can beat -- the exact area of the union of a block's
+    eight shifted 64 x 30 windows, rasterised here independently of the planner."""
+    cfg = synth.config(3)
+    times = synth.make_times(cfg, np.random.default_rng(cfg.seed))
+    vel = synth.velocity_grid(cfg.n_angles, cfg.n_speeds, cfg.ang_lo, cfg.ang_hi, cfg.speed_lo, cfg.speed_hi)
+    fills = {}
+    for geom in (0, 1):
+        stream, shapes, info = binding.debug_staged_plan(times, cfg.N, cfg.H, cfg.W, vel, geom)
+        tma = stream[(stream[:, 0] & 0xFF) == 1]
+        bw, bh = tma[:, 4] & 0xFFFF, tma[:, 4] >> 16
+        assert (bw * bh <= info["CAP"]).all() and (bw % 2 == 0).all()
+        fills[geom] = float((bw.astype(np.int64) * bh).sum()) / (cfg.V * cfg.N * info["TW"] * info["TH"])
+        order = stream[(stream[:, 0] >> 8) & 1 == 1][:, 8 + info["B"]:8 + 2 * info["B"]]      # velocities of every block
+    assert 0.66 < fills[1] < fills[0] < 0.72, fills            # 0.675 (cap 6144) and 0.692 (cap 4096)
+    # exact union of the windows of every block and image (image 0 is read once per block: not staged)
+    dt = (times - times[0]).astype(np.float32)
+    sh = np.floor(vel[:, None, :].astype(np.float64) * dt[None, :, None] + 0.5).astype(np.int64)
+    TW, TH = info["TW"], info["TH"]
+    union = 0
+    for blk in order:
+        js = blk[blk >= 0]
+        for i in range(1, cfg.N):
+            s = sh[js, i]
+            x0, y0 = s[:, 0].min(), s[:, 1].min()
+            g = np.zeros((s[:, 1].max() - y0 + TH, s[:, 0].max() - x0 + TW), bool)
+            for sx, sy in s:
+                g[sy - y0:sy - y0 + TH, sx - x0:sx - x0 + TW] = True
+            union += int(g.sum())
+    floor = union / (cfg.V * cfg.N * TW * TH)
+    assert 0.55 < floor < 0.59, floor                          # 0.570: no plan of 64 x 30 x 8 blocks stages less
+    assert fills[1] / floor < 1.25
