@@ -104,4 +104,12 @@ unsigned long long simt_selftest_ldg_past_end(int past) {
     return __ldg(b.as<const unsigned long long>() + 7 + past);
 }
 
+// Detector self-test: a float4 load `misalign` bytes off a 16-byte boundary, inside the buffer.
+// misalign = 0 is legal; 4 or 8 is a misaligned-address fault on the GPU and must abort under UBSan.
+float simt_selftest_ldg128_misaligned(int misalign) {
+    simt::DevBuf b(64, 256, 0);
+    const float4 v = __ldg(reinterpret_cast<const float4*>(b.as<char>() + 16 + misalign));
+    return v.x + v.w;
+}
+
 }  // extern "C"

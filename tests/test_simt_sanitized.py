@@ -95,3 +95,22 @@ def test_the_detector_detects():
     bad = subprocess.run([sys.executable, "-c", code, "1"], cwd=ROOT, env=env, capture_output=True, text=True)
     assert bad.returncode != 0 and "survived" not in bad.stdout
     assert "heap-buffer-overflow" in bad.stderr
+
+
+def test_the_detector_detects_misaligned_vector_loads():
+    """A 16-byte vector load 4 or 8 bytes off its alignment (a "misaligned address" fault on the GPU)
+    aborts the sanitized child with UBSan's misaligned-address report; an aligned one does not."""
+    rt = _asan_runtime()
+    if rt is None:
+        pytest.skip("gcc has no libasan.so on this machine")
+    env = dict(os.environ, LD_PRELOAD=rt, KBMOD_SIMT_SANITIZE="1", ASAN_OPTIONS="detect_leaks=0",
+               UBSAN_OPTIONS="print_stacktrace=1:halt_on_error=1")
+    code = ("import ctypes, sys; from tests import simt_build; L = simt_build.load('tiled_simt'); "
+            "L.simt_selftest_ldg128_misaligned.restype = ctypes.c_float; "
+            "L.simt_selftest_ldg128_misaligned(int(sys.argv[1])); print('survived')")
+    ok = subprocess.run([sys.executable, "-c", code, "0"], cwd=ROOT, env=env, capture_output=True, text=True)
+    assert ok.returncode == 0 and "survived" in ok.stdout, ok.stderr[-2000:]
+    for off in ("4", "8"):
+        bad = subprocess.run([sys.executable, "-c", code, off], cwd=ROOT, env=env, capture_output=True, text=True)
+        assert bad.returncode != 0 and "survived" not in bad.stdout, off
+        assert "misaligned address" in bad.stderr, bad.stderr[-1500:]
