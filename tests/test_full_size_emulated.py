@@ -61,6 +61,8 @@ def test_bands_of_the_full_size_stack(stack, reference, kernel):
 
 
 @pytest.mark.parametrize("name,k,over,bands", [
+    # BASELINE.json configs[1]: 8 x 2048 x 4096 (H < W), V = 512
+    ("config2", 2, {}, ((0, 32), (1016, 1048), (2040, 2048))),
     # BASELINE.json configs[3]: K = 16 (64 x 16 tiles, blocks of 16), V = 2048, irregular times, N = 12
     ("config4", 4, {}, ((0, 16), (2048, 2064), (4088, 4096))),
     # configs[4], the far corners of the sweep: N = 40 (additive counters, 5.4 GB stack) and V = 8192
@@ -79,3 +81,38 @@ def test_bands_of_the_other_full_size_configs(orc, name, k, over, bands, kernel)
                         T.QUEUED if kernel == "queued" else T.TILED, order=0, y_begin=y0, y_end=y1)
         T.assert_exact(out, ref)
         print(f"{name} {kernel} rows [{y0}, {y1}): bit-exact, {time.time() - t:.0f} s", flush=True)
+
+
+def test_staged_kernel_band_of_config4(orc):
+    """Kernel 3 at BASELINE.json configs[3]: K = 16 (generic list insert), V = 2048, irregular times."""
+    cfg = synth.config(4)
+    times, vel = _grid(cfg)
+    pp = synth.random_psiphi(cfg.N, cfg.H, cfg.W, seed=44, invalid_frac=0.1)
+    y0, y1 = 2040, 2070                                   # one 30-row tile row in the interior
+    t = time.time()
+    ref = orc.search(pp, times, vel, cfg.K, cfg.min_obs, y_begin=y0, y_end=y1)
+    rc, out, stats = S.run_sim(simt_build.load("staged_simt"), pp, times, vel, cfg.K, cfg.min_obs, order=0, sms=8,
+                               y_begin=y0, y_end=y1)
+    S.assert_exact(out, ref, stats, rc)
+    print(f"config4 staged rows [{y0}, {y1}): bit-exact, {time.time() - t:.0f} s", flush=True)
+
+
+def test_psi_phi_on_full_size_images(orc):
+    """kbmod_make_psi_phi's one-launch kernel on two full 4096 x 4096 images of configs[2] (P = 21;
+    8 192 tiles per image, the image index decoded from blockIdx.x): bands of rows at the top edge, at
+    a tile seam and at the bottom edge against the oracle run on the same rows plus the PSF halo."""
+    import ctypes
+    from tests.test_post_simt import assert_psiphi_close, run_psi_phi
+    cfg = synth.config(3, N=2, n_sources=50)
+    st = synth.make_stack(cfg)
+    t = time.time()
+    got, launches = run_psi_phi(simt_build.load("post_simt"), st.sci, st.var, st.mask, st.psf)
+    assert launches == 1
+    print(f"psi/phi of 2 x 4096 x 4096 emulated in {time.time() - t:.0f} s", flush=True)
+    r = (st.psf.shape[-1] - 1) // 2
+    for y0 in (0, 28, 2044, cfg.H - 8):
+        a, b = max(0, y0 - r), min(cfg.H, y0 + 8 + r)
+        ref, pabs = orc.make_psi_phi(st.sci[:, a:b], st.var[:, a:b], st.mask[:, a:b], st.psf, want_abs=True)
+        sl = slice(y0 - a, y0 - a + 8)
+        assert_psiphi_close(got[:, y0:y0 + 8], ref[:, sl], pabs[:, sl])
+    assert np.isnan(got[..., 0]).mean() > 0.005          # the 1 % mask is there
