@@ -124,3 +124,60 @@ def test_no_cpu_fallback_without_device(L):
     p = ctypes.c_void_p((buf.ctypes.data + 255) // 256 * 256)
     one = np.ones(1, np.float32).ctypes.data_as(ctypes.c_void_p)
     assert L.kbmod_make_psi_phi(p, p, None, one, 1, 2, 2, 1, p, None) == -5
+
+
+def test_next_row_calls_reject_bad_arguments_before_any_launch(L):
+    """kbmod_search_threshold / kbmod_filter_candidates / kbmod_coadd_stamps / kbmod_build_mask /
+    kbmod_cluster_candidates: every argument error has its code and is found before a device is
+    needed (no GPU here: a call that passes all checks returns KBMOD_ERR_CUDA = -5)."""
+    import torch
+    f = np.zeros(256, np.float32)
+    buf = np.zeros(8192, np.uint8)
+    fp = ctypes.c_void_p((f.ctypes.data + 15) // 16 * 16)
+    ws = ctypes.c_void_p((buf.ctypes.data + 255) // 256 * 256)
+    t = np.array([0.0, 1.0]).ctypes.data_as(ctypes.c_void_p)
+    bad_t = np.array([0.0, np.nan]).ctypes.data_as(ctypes.c_void_p)
+    vel = np.ones(2, np.float32).ctypes.data_as(ctypes.c_void_p)
+    big = ctypes.c_size_t(1 << 40)
+    cf = ctypes.c_float
+    no_gpu = -5 if not torch.cuda.is_available() else 0
+
+    class C(ctypes.Structure):
+        _fields_ = [(n, ctypes.c_void_p) for n in ("x", "y", "v", "n", "psi", "phi", "nu", "alpha")]
+    c = C(*[f.ctypes.data] * 8)
+    thr = lambda mo=1, nu=cf(5.0), y0=0, y1=4, cap=4, cnt=fp, opt=None, wsb=big: L.kbmod_search_threshold(
+        fp, t, 2, 4, 4, vel, 1, mo, nu, y0, y1, ctypes.byref(c), ctypes.c_longlong(cap), cnt, ws, wsb, opt, None)
+    assert thr(mo=3) == -3 and thr(nu=cf(float("nan"))) == -3 and thr(y0=3, y1=2) == -3 and thr(cap=-1) == -3
+    assert thr(cnt=None) == -1 and thr(wsb=ctypes.c_size_t(16)) == -7
+
+    class O(ctypes.Structure):
+        _fields_ = [(n, ctypes.c_int32) for n in ("struct_size", "kernel", "tile_group_w", "staged_geom")]
+    assert thr(opt=ctypes.byref(O(16, 2, 0, 0))) == -6 and thr(opt=ctypes.byref(O(16, 3, 0, 0))) == -6   # top-K only kernels
+    if no_gpu:
+        assert thr() == no_gpu and thr(opt=ctypes.byref(O(16, 4, 0, 0))) == no_gpu
+
+    filt = lambda N=2, M=1, s=cf(5.0), q=cf(0.0), tt=t, xy=fp: L.kbmod_filter_candidates(
+        fp, tt, N, 4, 4, xy, fp, M, s, q, fp, fp, fp, fp, fp, fp, None, None)
+    assert filt(N=65) == -6 and filt(N=0) == -2 and filt(M=-1) == -2 and filt(s=cf(0.0)) == -3
+    assert filt(q=cf(-1.0)) == -3 and filt(tt=bad_t) == -3 and filt(xy=None) == -1
+    if no_gpu:
+        assert filt() == no_gpu
+
+    stamps = lambda R=3, M=1, N=2: L.kbmod_coadd_stamps(fp, None, t, N, 4, 4, fp, fp, None, M, R, fp, None, None)
+    assert stamps(R=-1) == -3 and stamps(R=16) == -6 and stamps(N=65) == -6 and stamps(M=-2) == -2
+    if no_gpu:
+        assert stamps() == no_gpu
+
+    mask = lambda grow=2, mi=2, out=fp: L.kbmod_build_mask(fp, fp, None, 2, 4, 4, cf(5.0), grow, mi, cf(120.0), out, None)
+    assert mask(grow=-1) == -3 and mask(grow=9) == -6 and mask(mi=0) == -3 and mask(out=None) == -1
+    if no_gpu:
+        assert mask() == no_gpu
+
+    L.kbmod_cluster_workspace.restype = ctypes.c_size_t
+    assert L.kbmod_cluster_workspace(1000) >= 1000 * 9 and L.kbmod_cluster_workspace(-1) == 0
+    clus = lambda M=4, exy=cf(2.0), ev=cf(4.0), ms=1, wsb=big: L.kbmod_cluster_candidates(
+        fp, fp, fp, M, exy, ev, ms, fp, fp, ws, wsb, None)
+    assert clus(M=-1) == -2 and clus(exy=cf(0.0)) == -3 and clus(ev=cf(float("inf"))) == -3 and clus(ms=0) == -3
+    assert clus(wsb=ctypes.c_size_t(8)) == -7
+    if no_gpu:
+        assert clus() == no_gpu and clus(M=0) == no_gpu
